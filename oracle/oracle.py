@@ -1,0 +1,168 @@
+"""ctypes/numpy wrapper of the CPU oracle (oracle/chefsi_oracle.c).  TEST INFRASTRUCTURE, NOT PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this.  The product package (paper_2302_09708_b200) never imports it, and this module never imports
+the product's CUDA binding; the only shared module is the seeded input generator
+``paper_2302_09708_b200.workloads`` (inputs only).
+
+Two builds of the same source:
+  liboracle_ld.so   acc_t = long double   (parity oracle)
+  liboracle_f64.so  acc_t = double        (plain-FP64 CPU baseline that bench.py times)
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+import threading
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "chefsi_oracle.c")
+_LOCK = threading.Lock()
+_LIBS = {}
+
+
+def build(force: bool = False) -> None:
+    """Compile both oracle builds with gcc (-O3 -march=native -fopenmp)."""
+    for tag, extra in (("ld", []), ("f64", ["-DORACLE_ACC_DOUBLE"])):
+        out = os.path.join(_HERE, f"liboracle_{tag}.so")
+        if (not force and os.path.exists(out)
+                and os.path.getmtime(out) >= os.path.getmtime(_SRC)):
+            continue
+        cmd = ["gcc", "-O3", "-march=native", "-fopenmp", "-fPIC", "-shared", "-std=c11",
+               "-fno-fast-math", *extra, _SRC, "-o", out + ".tmp", "-lm"]
+        subprocess.check_call(cmd)
+        os.replace(out + ".tmp", out)
+
+
+class _Ham(C.Structure):
+    _fields_ = [("n", C.c_int32 * 3), ("h", C.c_double * 3), ("bc", C.c_int32 * 3),
+                ("radius", C.c_int32), ("n_atoms", C.c_int32),
+                ("supp_ptr", C.c_void_p), ("supp_idx", C.c_void_p), ("n_proj", C.c_void_p),
+                ("chi_ptr", C.c_void_p), ("chi", C.c_void_p), ("gamma", C.c_void_p),
+                ("veff", C.c_void_p)]
+
+
+def _lib(acc: str = "ld"):
+    with _LOCK:
+        if acc not in _LIBS:
+            build()
+            lib = C.CDLL(os.path.join(_HERE, f"liboracle_{acc}.so"))
+            P, I64, D = C.c_void_p, C.c_int64, C.c_double
+            lib.oracle_acc_bits.restype = C.c_int
+            lib.oracle_fd_weights.argtypes = [C.c_int, P]
+            for name in ("oracle_laplacian", "oracle_vnl_apply", "oracle_h_apply"):
+                getattr(lib, name).argtypes = [C.POINTER(_Ham), P, I64, P, I64, I64]
+                getattr(lib, name).restype = None
+            lib.oracle_chebyshev_filter.argtypes = [C.POINTER(_Ham), P, I64, I64, C.c_int, D, D, D]
+            lib.oracle_chebyshev_filter.restype = C.c_int
+            lib.oracle_gram.argtypes = [P, I64, P, I64, I64, P, I64, P, I64, P]
+            lib.oracle_gram.restype = None
+            lib.oracle_rotate.argtypes = [P, I64, I64, P, P, I64, P]
+            lib.oracle_rotate.restype = None
+            _LIBS[acc] = lib
+        return _LIBS[acc]
+
+
+def _ptr(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _fcols(x: np.ndarray) -> np.ndarray:
+    x = np.asarray(x, dtype=np.float64)
+    if x.ndim == 1:
+        x = x.reshape(-1, 1)
+    return np.asfortranarray(x)
+
+
+class Hamiltonian:
+    """Holds the (host) description of H for the oracle.  `wl` is a workloads.Workload-like object
+    (attributes n, h, bc, fd_order, supp_ptr, supp_idx, n_proj, chi_ptr, chi, gamma, veff)."""
+
+    def __init__(self, wl, acc: str = "ld", nonlocal_on: bool = True):
+        self.lib = _lib(acc)
+        self.nd = int(wl.n[0]) * int(wl.n[1]) * int(wl.n[2])
+        self._keep = dict(
+            supp_ptr=np.ascontiguousarray(wl.supp_ptr, dtype=np.int64),
+            supp_idx=np.ascontiguousarray(wl.supp_idx, dtype=np.int32),
+            n_proj=np.ascontiguousarray(wl.n_proj, dtype=np.int32),
+            chi_ptr=np.ascontiguousarray(wl.chi_ptr, dtype=np.int64),
+            chi=np.ascontiguousarray(wl.chi, dtype=np.float64),
+            gamma=np.ascontiguousarray(wl.gamma, dtype=np.float64),
+            veff=np.ascontiguousarray(wl.veff, dtype=np.float64))
+        assert self._keep["veff"].shape[0] == self.nd
+        h = _Ham()
+        for k in range(3):
+            h.n[k] = int(wl.n[k]); h.h[k] = float(wl.h[k]); h.bc[k] = int(wl.bc[k])
+        h.radius = int(wl.fd_order) // 2
+        h.n_atoms = int(self._keep["n_proj"].shape[0]) if nonlocal_on else 0
+        for name in ("supp_ptr", "supp_idx", "n_proj", "chi_ptr", "chi", "gamma", "veff"):
+            setattr(h, name, self._keep[name].ctypes.data)
+        self.h = h
+
+    def _apply(self, fn, X):
+        X = _fcols(X)
+        assert X.shape[0] == self.nd
+        Y = np.empty_like(X, order="F")
+        fn(C.byref(self.h), _ptr(X), X.shape[0], _ptr(Y), Y.shape[0], X.shape[1])
+        return Y
+
+    def laplacian(self, X):            # O2
+        return self._apply(self.lib.oracle_laplacian, X)
+
+    def vnl_apply(self, X):            # O4
+        return self._apply(self.lib.oracle_vnl_apply, X)
+
+    def apply(self, X):                # O5
+        return self._apply(self.lib.oracle_h_apply, X)
+
+    def chebyshev_filter(self, X, degree: int, a: float, b: float, a0: float):   # O6
+        Y = _fcols(X).copy(order="F")
+        rc = self.lib.oracle_chebyshev_filter(C.byref(self.h), _ptr(Y), Y.shape[0], Y.shape[1],
+                                              int(degree), float(a), float(b), float(a0))
+        if rc != 0:
+            raise ValueError(f"oracle_chebyshev_filter: bad arguments (rc={rc})")
+        return Y
+
+    def project(self, Psi):            # O7
+        Psi = _fcols(Psi)
+        Y = self.apply(Psi)
+        return gram(Psi, Y, lib=self.lib), gram(Psi, Psi, lib=self.lib)
+
+
+def fd_weights(radius: int) -> np.ndarray:   # O1
+    w = np.zeros(radius + 1)
+    _lib("ld").oracle_fd_weights(int(radius), _ptr(w))
+    return w
+
+
+def gram(A, B, I: Optional[Sequence[int]] = None, J: Optional[Sequence[int]] = None, lib=None,
+         acc: str = "ld") -> np.ndarray:
+    """out[i,j] = sum_r A[r, I[i]] B[r, J[j]]   (O7)."""
+    lib = lib or _lib(acc)
+    A, B = _fcols(A), _fcols(B)
+    assert A.shape[0] == B.shape[0]
+    Ia = None if I is None else np.ascontiguousarray(I, dtype=np.int64)
+    Ja = None if J is None else np.ascontiguousarray(J, dtype=np.int64)
+    nI = A.shape[1] if Ia is None else Ia.shape[0]
+    nJ = B.shape[1] if Ja is None else Ja.shape[0]
+    out = np.empty((nI, nJ), dtype=np.float64, order="F")
+    lib.oracle_gram(_ptr(A), A.shape[0], _ptr(B), B.shape[0], A.shape[0], _ptr(Ia), nI, _ptr(Ja), nJ,
+                    _ptr(out))
+    return out
+
+
+def rotate(Psi, Q, rows: Optional[Sequence[int]] = None, acc: str = "ld") -> np.ndarray:
+    """out[k,:] = Psi[rows[k],:] @ Q   (O8)."""
+    lib = _lib(acc)
+    Psi, Q = _fcols(Psi), _fcols(Q)
+    ns = Psi.shape[1]
+    assert Q.shape == (ns, ns)
+    R = None if rows is None else np.ascontiguousarray(rows, dtype=np.int64)
+    nrows = Psi.shape[0] if R is None else R.shape[0]
+    out = np.empty((nrows, ns), dtype=np.float64, order="F")
+    lib.oracle_rotate(_ptr(Psi), Psi.shape[0], ns, _ptr(Q), _ptr(R), nrows, _ptr(out))
+    return out
