@@ -1,0 +1,144 @@
+/*
+ * sparc_gpu.h -- C-ABI boundary of the B200-native CheFSI hot path (arxiv 2302.09708).
+ *
+ * What the library computes (citations are /root/reference/PAPER.md line numbers; "R<n>" are the
+ * readings listed in DESIGN.md section 3):
+ *
+ *   H = -1/2 Laplacian + Veff + V_nl, applied matrix-free to a block of N_s FP64 orbitals on a uniform
+ *   3-D grid of N_d = nx*ny*nz nodes (Algorithm 1, 102, 122).  The Laplacian is the
+ *   central finite-difference stencil of order n0 (3*n0+1 taps), periodic or Dirichlet
+ *   per axis; Veff multiplies pointwise; V_nl = sum_J S_J^T chi_J
+ *   diag(gamma_J) chi_J^T S_J applies each atom's dense projector matrix to "the appropriate
+ *   components" of the orbitals.  On top of H:
+ *     - the Chebyshev filter  X <- p_m((H - cI)/e) X
+ *     - the projection        Hs = X^T H X,  Ms = X^T X
+ *     - the rotation          X <- X Q   (Q = eigenvectors supplied by the caller; the N_s x N_s
+ *                             eigensolve, is outside this library)
+ *
+ * Conventions
+ *   - Real FP64 only (Gamma point).  Grid linear index i = x + nx*(y + ny*z).
+ *   - Psi, X, Y: N_d x ncols, column-major, leading dimension ld >= N_d; one column = one orbital.
+ *     Hs, Ms, Q: ns x ns, column-major, ld = ns.
+ *   - Pointers named *_dev are DEVICE pointers owned by the caller (e.g. PyTorch tensors); pointers in
+ *     sparc_gpu_desc are HOST pointers, copied at create (the caller may free them afterwards).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Every compute call
+ *     is asynchronous on `stream`, never synchronises the device and never touches host memory.
+ *   - `ws_dev` is caller-owned device scratch of at least sparc_gpu_workspace_bytes(...) bytes, 256-byte
+ *     aligned.  The library allocates only its immutable tables (weights, chi, index maps, Veff copy).
+ *   - Every call returns 0 on success or a negative sparc_gpu_status.  No exceptions, no exit(), no
+ *     printing.  There is NO CPU fallback: without an sm_100 device create fails with UNSUPPORTED.
+ */
+#ifndef SPARC_GPU_H
+#define SPARC_GPU_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sparc_gpu_ctx sparc_gpu_ctx;   /* opaque, owned by the library */
+
+typedef enum {
+    SPARC_GPU_SUCCESS = 0,
+    SPARC_GPU_INVALID_ARG = -1,         /* NULL pointer, negative size, ld < N_d, degree < 0, bad op ...  */
+    SPARC_GPU_UNSUPPORTED = -2,         /* fd_order not even in 2..12; periodic axis with n < n0+1 (R10);
+                                           device is not compute capability 10.x                            */
+    SPARC_GPU_BAD_BOUNDS = -3,          /* filter bounds must satisfy a0 < a < b (R5)                       */
+    SPARC_GPU_BAD_DESCRIPTOR = -4,      /* support index out of range / not strictly ascending within an
+                                           atom, inconsistent chi_ptr / supp_ptr, n_proj < 0 or > 16        */
+    SPARC_GPU_WORKSPACE_TOO_SMALL = -5, /* reserved: reported by bindings that know the size they passed    */
+    SPARC_GPU_OUT_OF_MEMORY = -6,       /* device allocation of the library's tables failed                 */
+    SPARC_GPU_CUDA_ERROR = -7           /* any other CUDA runtime / driver error                            */
+} sparc_gpu_status;
+
+typedef enum {
+    SPARC_GPU_OP_HAMILTONIAN_APPLY = 0,
+    SPARC_GPU_OP_CHEBYSHEV_FILTER = 1,
+    SPARC_GPU_OP_PROJECT = 2,
+    SPARC_GPU_OP_ROTATE = 3
+} sparc_gpu_op;
+
+/* Problem description (all pointers HOST, copied at create).  PAPER.md:118 "The matrix X, effective
+ * potential, and nonlocal projectors are then transferred from the host CPU to its mapped GPU". */
+typedef struct {
+    int32_t n[3];             /* nx, ny, nz                                                         */
+    double h[3];              /* grid spacing per axis, bohr (R17)                                  */
+    int32_t bc[3];            /* 0 = periodic, 1 = Dirichlet: psi = 0 outside [0, n-1] (R9)         */
+    int32_t fd_order;         /* n0: even, 2..12; stencil radius n0/2 (R1)            */
+    int32_t n_atoms;          /* may be 0 (no nonlocal term)                                        */
+    const int64_t *supp_ptr;  /* [n_atoms+1] offsets into supp_idx                                  */
+    const int32_t *supp_idx;  /* grid linear indices, strictly ascending within an atom (R8)        */
+    const int32_t *n_proj;    /* [n_atoms] number of projectors P_J of atom J (0..16)               */
+    const int64_t *chi_ptr;   /* [n_atoms+1] offsets (in doubles) into chi; atom J owns n_J*P_J     */
+    const double *chi;        /* per atom: n_J x P_J, column-major ("dense matrix")    */
+    const double *gamma;      /* concatenated P_J Kleinman-Bylander energies per atom (R6, R7)      */
+    const double *veff;       /* [N_d] or NULL (then set later with sparc_gpu_set_veff; zero until) */
+    int32_t device;           /* CUDA device ordinal                                                */
+} sparc_gpu_desc;
+
+/* Create a context on desc->device: validates the descriptor, uploads it, builds the stencil
+ * coefficient tables and the point -> (atom, row) inverse map used by the nonlocal pull kernel. */
+int sparc_gpu_create(const sparc_gpu_desc *desc, sparc_gpu_ctx **out);
+int sparc_gpu_destroy(sparc_gpu_ctx *ctx);
+
+/* New effective potential for the next SCF iteration: copies N_d doubles from
+ * veff_dev into the context's own buffer, asynchronously on `stream`. */
+int sparc_gpu_set_veff(sparc_gpu_ctx *ctx, const double *veff_dev, void *stream);
+
+/* Scratch needed by `op` on `ns` columns.  `block` is the column block (apply, filter, project) or the
+ * row panel (rotate) the call will be given; <= 0 means "library chooses" (query with the same value
+ * you will pass to the call). */
+int sparc_gpu_workspace_bytes(const sparc_gpu_ctx *ctx, int op, int64_t ns, int64_t block,
+                              int64_t *bytes);
+
+/* Y = H X on ncols columns (eq. 4, 122-126).  X and Y must not overlap.
+ * ldx, ldy >= N_d.  X is not modified. */
+int sparc_gpu_hamiltonian_apply(sparc_gpu_ctx *ctx, const double *X_dev, int64_t ldx, double *Y_dev,
+                                int64_t ldy, int64_t ncols, void *ws_dev, void *stream);
+
+/* In-place scaled Chebyshev filter (three-term scaled recurrence of refs [61,62], R3):
+ *   e = (b-a)/2, c = (b+a)/2, sigma_1 = e/(a0-c), tau = 2/sigma_1,
+ *   Y_1 = (sigma_1/e)(H X - c X);  Y_{k+1} = (2 sigma_{k+1}/e)(H Y_k - c Y_k) - sigma_k sigma_{k+1} Y_{k-1},
+ *   sigma_{k+1} = 1/(tau - sigma_k);   Psi <- Y_degree  ( = T_m((H-cI)/e) Psi / T_m((a0-c)/e) ).
+ * b = upper bound of the spectrum (lambda_Nd), a = filter cutoff (lambda_c), a0 = lower bound; requires
+ * a0 < a < b (BAD_BOUNDS).  degree = 0 is the identity, degree < 0 INVALID_ARG (R4).  Columns are
+ * processed in blocks of `col_block` (<= 0: library chooses); the result does not depend on it (R19). */
+int sparc_gpu_chebyshev_filter(sparc_gpu_ctx *ctx, double *Psi_dev, int64_t ld, int64_t ns, int degree,
+                               double a, double b, double a0, int64_t col_block, void *ws_dev,
+                               void *stream);
+
+/* Hs = Psi^T (H Psi), Ms = Psi^T Psi (R11: H Psi is formed internally by
+ * column blocks).  Both outputs are full ns x ns matrices with both triangles filled (R12). */
+int sparc_gpu_project(sparc_gpu_ctx *ctx, const double *Psi_dev, int64_t ld, int64_t ns, double *Hs_dev,
+                      double *Ms_dev, int64_t col_block, void *ws_dev, void *stream);
+
+/* Psi <- Psi Q in place, by row panels of `row_panel` rows (<= 0: library chooses) staged through the
+ * workspace.  The result does not depend on row_panel (R19). */
+int sparc_gpu_rotate(sparc_gpu_ctx *ctx, double *Psi_dev, int64_t ld, int64_t ns, const double *Q_dev,
+                     int64_t row_panel, void *ws_dev, void *stream);
+
+/* ---- support entry points (not operators of the method) ------------------------------------- */
+
+/* dst[k] = lo + (hi-lo) * u(seed, stream_id, index0 + k), k < count: the counter-based uniform generator
+ * of the synthetic workloads, restated on the device so that large Psi blocks never
+ * cross PCIe.  dst_dev is a device pointer. */
+int sparc_gpu_fill_uniform(double *dst_dev, int64_t count, uint64_t seed, uint64_t stream_id,
+                           uint64_t index0, double lo, double hi, int device, void *stream);
+
+/* Tuning / test knobs.  key: "stencil_path" (0 auto, 1 generic kernel, 2 TMA kernel or UNSUPPORTED),
+ * "nonlocal" (1 on, 0 off: drops V_nl, used by closed-form pins), "gemm_path" (0 auto, 1 simple FMA
+ * kernel, 2 DMMA kernel).  Unknown key -> INVALID_ARG. */
+int sparc_gpu_set_option(sparc_gpu_ctx *ctx, const char *key, int64_t value);
+
+/* Read-only counters / facts.  key: "kernel_launches" (cumulative kernels launched by this context),
+ * "nd", "n_proj_total", "covered_points", "stencil_path_last" (1 generic, 2 TMA), "sm_count". */
+int sparc_gpu_get_info(const sparc_gpu_ctx *ctx, const char *key, int64_t *value);
+
+const char *sparc_gpu_error_string(int code);
+const char *sparc_gpu_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPARC_GPU_H */

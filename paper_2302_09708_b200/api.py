@@ -1,0 +1,243 @@
+"""Thin Python binding of the sparc_gpu C-ABI library (include/sparc_gpu.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI; PyTorch is used here for device
+memory (tensors, workspaces) and streams only.  There is no CPU fallback: if libsparc_gpu.so cannot be
+loaded (and cannot be built), importing/using this module raises.
+
+Matrix convention: an N_d x ncols column-major matrix with leading dimension ld is held as a torch
+float64 CUDA tensor of shape (ncols, ld) that is contiguous along its last axis (so `t[j, :N_d]` is
+column j).  Helpers `colmajor_from_numpy` / `colmajor_to_numpy` convert from / to Fortran-ordered numpy.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libsparc_gpu.so")
+_lib = None
+
+OP_HAMILTONIAN_APPLY, OP_CHEBYSHEV_FILTER, OP_PROJECT, OP_ROTATE = 0, 1, 2, 3
+
+EXPORTS = ["sparc_gpu_create", "sparc_gpu_destroy", "sparc_gpu_set_veff", "sparc_gpu_workspace_bytes",
+           "sparc_gpu_hamiltonian_apply", "sparc_gpu_chebyshev_filter", "sparc_gpu_project",
+           "sparc_gpu_rotate", "sparc_gpu_fill_uniform", "sparc_gpu_set_option", "sparc_gpu_get_info",
+           "sparc_gpu_error_string", "sparc_gpu_version"]
+
+
+class SparcGpuError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        msg = load_library().sparc_gpu_error_string(code).decode()
+        super().__init__(f"{where}: {msg} (status {code})")
+
+
+class Desc(C.Structure):
+    _fields_ = [("n", C.c_int32 * 3), ("h", C.c_double * 3), ("bc", C.c_int32 * 3),
+                ("fd_order", C.c_int32), ("n_atoms", C.c_int32),
+                ("supp_ptr", C.c_void_p), ("supp_idx", C.c_void_p), ("n_proj", C.c_void_p),
+                ("chi_ptr", C.c_void_p), ("chi", C.c_void_p), ("gamma", C.c_void_p),
+                ("veff", C.c_void_p), ("device", C.c_int32)]
+
+
+def load_library(build_if_missing: bool = True):
+    """dlopen libsparc_gpu.so (building it in-tree with nvcc if absent).  Raises if impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        if not build_if_missing:
+            raise RuntimeError(f"{_LIB_PATH} is missing: run `python -m paper_2302_09708_b200.build`")
+        from . import build as _build
+        _build.build()
+    lib = C.CDLL(_LIB_PATH)
+    P, I64, D, I = C.c_void_p, C.c_int64, C.c_double, C.c_int
+    lib.sparc_gpu_create.argtypes = [C.POINTER(Desc), C.POINTER(P)]
+    lib.sparc_gpu_destroy.argtypes = [P]
+    lib.sparc_gpu_set_veff.argtypes = [P, P, P]
+    lib.sparc_gpu_workspace_bytes.argtypes = [P, I, I64, I64, C.POINTER(I64)]
+    lib.sparc_gpu_hamiltonian_apply.argtypes = [P, P, I64, P, I64, I64, P, P]
+    lib.sparc_gpu_chebyshev_filter.argtypes = [P, P, I64, I64, I, D, D, D, I64, P, P]
+    lib.sparc_gpu_project.argtypes = [P, P, I64, I64, P, P, I64, P, P]
+    lib.sparc_gpu_rotate.argtypes = [P, P, I64, I64, P, I64, P, P]
+    lib.sparc_gpu_fill_uniform.argtypes = [P, I64, C.c_uint64, C.c_uint64, C.c_uint64, D, D, I, P]
+    lib.sparc_gpu_set_option.argtypes = [P, C.c_char_p, I64]
+    lib.sparc_gpu_get_info.argtypes = [P, C.c_char_p, C.POINTER(I64)]
+    lib.sparc_gpu_error_string.argtypes = [I]
+    lib.sparc_gpu_error_string.restype = C.c_char_p
+    lib.sparc_gpu_version.restype = C.c_char_p
+    for name in EXPORTS[:-2]:
+        getattr(lib, name).restype = I
+    _lib = lib
+    return lib
+
+
+def _check(code: int, where: str):
+    if code != 0:
+        raise SparcGpuError(code, where)
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _stream_ptr():
+    return C.c_void_p(_torch().cuda.current_stream().cuda_stream)
+
+
+def colmajor_from_numpy(a: np.ndarray, device="cuda", ld: Optional[int] = None):
+    """(rows x cols) numpy array -> torch (cols, ld) float64 CUDA tensor holding it column-major."""
+    torch = _torch()
+    a = np.asarray(a, dtype=np.float64)
+    if a.ndim == 1:
+        a = a.reshape(-1, 1)
+    rows, cols = a.shape
+    ld = rows if ld is None else int(ld)
+    t = torch.zeros((cols, ld), dtype=torch.float64, device=device)
+    t[:, :rows] = torch.from_numpy(np.ascontiguousarray(a.T)).to(device)
+    return t
+
+
+def colmajor_to_numpy(t, rows: Optional[int] = None) -> np.ndarray:
+    rows = t.shape[1] if rows is None else rows
+    return np.asfortranarray(t[:, :rows].detach().cpu().numpy().T)
+
+
+def fill_uniform(t, seed: int, stream_id: int, index0: int, lo: float, hi: float):
+    """t.view(-1)[k] = lo + (hi-lo)*u(seed, stream_id, index0+k) on the device (contiguous tensor)."""
+    assert t.is_cuda and t.is_contiguous() and t.dtype == _torch().float64
+    _check(load_library().sparc_gpu_fill_uniform(C.c_void_p(t.data_ptr()), t.numel(), seed, stream_id, index0,
+                                                 lo, hi, t.device.index or 0, _stream_ptr()), "fill_uniform")
+    return t
+
+
+class SparcGpu:
+    """One sparc_gpu context: H = -1/2 Laplacian + Veff + V_nl on a fixed grid (see include/sparc_gpu.h)."""
+
+    def __init__(self, wl, device: int = 0, upload_veff: bool = True):
+        """`wl`: object with attributes n, h, bc, fd_order, supp_ptr, supp_idx, n_proj, chi_ptr, chi, gamma,
+        veff (numpy arrays; e.g. workloads.Workload)."""
+        torch = _torch()
+        if not torch.cuda.is_available():
+            raise RuntimeError("sparc_gpu needs a CUDA device (no CPU fallback)")
+        self.lib = load_library()
+        self.device = int(device)
+        self.nd = int(wl.n[0]) * int(wl.n[1]) * int(wl.n[2])
+        keep = dict(
+            supp_ptr=np.ascontiguousarray(wl.supp_ptr, dtype=np.int64),
+            supp_idx=np.ascontiguousarray(wl.supp_idx, dtype=np.int32),
+            n_proj=np.ascontiguousarray(wl.n_proj, dtype=np.int32),
+            chi_ptr=np.ascontiguousarray(wl.chi_ptr, dtype=np.int64),
+            chi=np.ascontiguousarray(wl.chi, dtype=np.float64),
+            gamma=np.ascontiguousarray(wl.gamma, dtype=np.float64))
+        d = Desc()
+        for k in range(3):
+            d.n[k], d.h[k], d.bc[k] = int(wl.n[k]), float(wl.h[k]), int(wl.bc[k])
+        d.fd_order = int(wl.fd_order)
+        d.n_atoms = int(keep["n_proj"].shape[0])
+        for name, arr in keep.items():
+            setattr(d, name, arr.ctypes.data if arr.size else None)
+        veff = None
+        if upload_veff and getattr(wl, "veff", None) is not None:
+            veff = np.ascontiguousarray(wl.veff, dtype=np.float64)
+            assert veff.shape[0] == self.nd
+            d.veff = veff.ctypes.data
+        d.device = self.device
+        self._ctx = C.c_void_p()
+        torch.cuda.init()
+        _check(self.lib.sparc_gpu_create(C.byref(d), C.byref(self._ctx)), "sparc_gpu_create")
+        self._ws = None
+
+    # ---- lifetime -----------------------------------------------------------------------------
+    def close(self):
+        if getattr(self, "_ctx", None) is not None and self._ctx.value:
+            self.lib.sparc_gpu_destroy(self._ctx)
+            self._ctx = C.c_void_p()
+        self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- plumbing -----------------------------------------------------------------------------
+    def workspace_bytes(self, op: int, ns: int, block: int = 0) -> int:
+        out = C.c_int64()
+        _check(self.lib.sparc_gpu_workspace_bytes(self._ctx, op, ns, block, C.byref(out)), "workspace_bytes")
+        return out.value
+
+    def _workspace(self, op: int, ns: int, block: int):
+        torch = _torch()
+        need = self.workspace_bytes(op, ns, block)
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = None
+            self._ws = torch.empty(need, dtype=torch.uint8, device=f"cuda:{self.device}")
+        return C.c_void_p(self._ws.data_ptr())
+
+    def release_workspace(self):
+        self._ws = None
+
+    def set_option(self, key: str, value: int):
+        _check(self.lib.sparc_gpu_set_option(self._ctx, key.encode(), int(value)), f"set_option({key})")
+
+    def get_info(self, key: str) -> int:
+        out = C.c_int64()
+        _check(self.lib.sparc_gpu_get_info(self._ctx, key.encode(), C.byref(out)), f"get_info({key})")
+        return out.value
+
+    def _mat(self, t, name: str) -> Tuple[C.c_void_p, int, int]:
+        torch = _torch()
+        if not (t.is_cuda and t.dtype == torch.float64 and t.dim() == 2 and t.stride(1) == 1):
+            raise ValueError(f"{name}: need a 2-D float64 CUDA tensor (ncols, ld) contiguous along ld")
+        if t.shape[1] < self.nd:
+            raise ValueError(f"{name}: ld {t.shape[1]} < N_d {self.nd}")
+        return C.c_void_p(t.data_ptr()), int(t.stride(0)) if t.shape[0] > 1 else int(t.shape[1]), int(t.shape[0])
+
+    # ---- the C-ABI calls ----------------------------------------------------------------------
+    def set_veff(self, veff):
+        assert veff.is_cuda and veff.numel() >= self.nd and veff.is_contiguous()
+        _check(self.lib.sparc_gpu_set_veff(self._ctx, C.c_void_p(veff.data_ptr()), _stream_ptr()), "set_veff")
+
+    def hamiltonian_apply(self, X, Y=None):
+        torch = _torch()
+        xp, ldx, ncols = self._mat(X, "X")
+        if Y is None:
+            Y = torch.empty_like(X)
+        yp, ldy, _ = self._mat(Y, "Y")
+        ws = self._workspace(OP_HAMILTONIAN_APPLY, ncols, 0)
+        _check(self.lib.sparc_gpu_hamiltonian_apply(self._ctx, xp, ldx, yp, ldy, ncols, ws, _stream_ptr()),
+               "hamiltonian_apply")
+        return Y
+
+    def chebyshev_filter(self, Psi, degree: int, a: float, b: float, a0: float, col_block: int = 0):
+        pp, ld, ns = self._mat(Psi, "Psi")
+        ws = self._workspace(OP_CHEBYSHEV_FILTER, ns, col_block)
+        _check(self.lib.sparc_gpu_chebyshev_filter(self._ctx, pp, ld, ns, int(degree), float(a), float(b),
+                                                   float(a0), int(col_block), ws, _stream_ptr()),
+               "chebyshev_filter")
+        return Psi
+
+    def project(self, Psi, col_block: int = 0, Hs=None, Ms=None):
+        torch = _torch()
+        pp, ld, ns = self._mat(Psi, "Psi")
+        if Hs is None:
+            Hs = torch.empty((ns, ns), dtype=torch.float64, device=Psi.device)
+        if Ms is None:
+            Ms = torch.empty((ns, ns), dtype=torch.float64, device=Psi.device)
+        ws = self._workspace(OP_PROJECT, ns, col_block)
+        _check(self.lib.sparc_gpu_project(self._ctx, pp, ld, ns, C.c_void_p(Hs.data_ptr()),
+                                          C.c_void_p(Ms.data_ptr()), int(col_block), ws, _stream_ptr()), "project")
+        return Hs, Ms       # (ns, ns) tensors holding the column-major matrices: element [j, i] = M_ij
+
+    def rotate(self, Psi, Q, row_panel: int = 0):
+        pp, ld, ns = self._mat(Psi, "Psi")
+        assert Q.is_cuda and Q.shape == (ns, ns) and Q.is_contiguous()
+        ws = self._workspace(OP_ROTATE, ns, row_panel)
+        _check(self.lib.sparc_gpu_rotate(self._ctx, pp, ld, ns, C.c_void_p(Q.data_ptr()), int(row_panel), ws,
+                                         _stream_ptr()), "rotate")
+        return Psi

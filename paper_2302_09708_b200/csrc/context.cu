@@ -1,0 +1,424 @@
+// context.cu -- C-ABI entry points: context lifetime, validation, host-side orchestration of the
+// filter / project / rotate passes.  All arithmetic of the method runs in the kernels launched from
+// here (stencil_*.cu, nonlocal.cu, gemm.cu); this file only sequences them.
+#include <cuda.h>
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+#include <vector>
+
+#include "internal.h"
+
+namespace {
+
+// O(1) host arithmetic: central FD weights of the second derivative, radius r (R1).
+void fd_weights_host(int r, double *w)
+{
+    long double w0 = 0.0L;
+    for (int p = 1; p <= r; ++p) {
+        long double ratio = 1.0L;   // (r!)^2 / ((r-p)! (r+p)!)
+        for (int j = 1; j <= p; ++j) ratio *= (long double)(r - p + j) / (long double)(r + j);
+        long double v = 2.0L / ((long double)p * p) * ratio;
+        w[p] = (double)((p & 1) ? v : -v);
+        w0 -= 2.0L / ((long double)p * p);
+    }
+    w[0] = (double)w0;
+}
+
+template <typename T>
+int upload(T **dst, const T *src, size_t count)
+{
+    *dst = nullptr;
+    if (count == 0) return SPARC_GPU_SUCCESS;
+    SPARC_CUDA_TRY(cudaMalloc((void **)dst, count * sizeof(T)));
+    SPARC_CUDA_TRY(cudaMemcpy(*dst, src, count * sizeof(T), cudaMemcpyHostToDevice));
+    return SPARC_GPU_SUCCESS;
+}
+
+void free_tables(sparc_gpu_ctx *c)
+{
+    cudaFree(c->d_supp_ptr); cudaFree(c->d_supp_idx); cudaFree(c->d_n_proj); cudaFree(c->d_proj_ofs);
+    cudaFree(c->d_chi_ptr); cudaFree(c->d_chi); cudaFree(c->d_gamma); cudaFree(c->d_cov_idx);
+    cudaFree(c->d_cov_ptr); cudaFree(c->d_cov_ent); cudaFree(c->d_veff);
+}
+
+int validate_desc(const sparc_gpu_desc *d)
+{
+    for (int a = 0; a < 3; ++a) {
+        if (d->n[a] < 1 || !(d->h[a] > 0.0) || !std::isfinite(d->h[a])) return SPARC_GPU_INVALID_ARG;
+        if (d->bc[a] != 0 && d->bc[a] != 1) return SPARC_GPU_INVALID_ARG;
+    }
+    if ((int64_t)d->n[0] * d->n[1] * d->n[2] >= (int64_t)INT32_MAX) return SPARC_GPU_UNSUPPORTED;   // R20
+    if (d->fd_order < 2 || d->fd_order > 2 * SPARC_MAX_RADIUS || (d->fd_order & 1)) return SPARC_GPU_UNSUPPORTED;
+    for (int a = 0; a < 3; ++a)
+        if (d->bc[a] == 0 && d->n[a] < d->fd_order + 1) return SPARC_GPU_UNSUPPORTED;               // R10
+    if (d->n_atoms < 0) return SPARC_GPU_INVALID_ARG;
+    if (d->n_atoms > 0) {
+        if (!d->supp_ptr || !d->supp_idx || !d->n_proj || !d->chi_ptr || !d->chi || !d->gamma)
+            return SPARC_GPU_INVALID_ARG;
+        const int64_t nd = (int64_t)d->n[0] * d->n[1] * d->n[2];
+        if (d->supp_ptr[0] != 0 || d->chi_ptr[0] != 0) return SPARC_GPU_BAD_DESCRIPTOR;
+        for (int J = 0; J < d->n_atoms; ++J) {
+            const int64_t s0 = d->supp_ptr[J], s1 = d->supp_ptr[J + 1];
+            const int P = d->n_proj[J];
+            if (s1 < s0 || P < 0 || P > SPARC_MAX_PROJ) return SPARC_GPU_BAD_DESCRIPTOR;
+            if (d->chi_ptr[J + 1] - d->chi_ptr[J] != (s1 - s0) * P) return SPARC_GPU_BAD_DESCRIPTOR;
+            for (int64_t t = s0; t < s1; ++t) {
+                const int32_t i = d->supp_idx[t];
+                if (i < 0 || i >= nd) return SPARC_GPU_BAD_DESCRIPTOR;
+                if (t > s0 && i <= d->supp_idx[t - 1]) return SPARC_GPU_BAD_DESCRIPTOR;             // R8
+            }
+        }
+    }
+    return SPARC_GPU_SUCCESS;
+}
+
+struct WsLayout {
+    int64_t block;       // column block / row panel actually used
+    int64_t ldw;         // leading dimension of the work block
+    int64_t off_w, off_d, off_g;
+    int64_t total;
+};
+
+int64_t default_col_block(const sparc_gpu_ctx *c, int64_t ns) { (void)c; return std::min<int64_t>(ns, 1024); }
+
+int64_t default_row_panel(const sparc_gpu_ctx *c, int64_t ns)
+{
+    // stage of at most ~2 GiB, at least 128 rows, multiple of 128
+    int64_t r = (int64_t)(2048LL << 20) / (8 * std::max<int64_t>(ns, 1));
+    r = std::max<int64_t>(128, r / 128 * 128);
+    return std::min<int64_t>(r, round_up_i64(c->nd, 128));
+}
+
+int ws_layout(const sparc_gpu_ctx *c, int op, int64_t ns, int64_t block, WsLayout *L)
+{
+    if (ns < 0) return SPARC_GPU_INVALID_ARG;
+    memset(L, 0, sizeof(*L));
+    const int64_t A = 256;
+    int64_t off = 0;
+    switch (op) {
+    case SPARC_GPU_OP_HAMILTONIAN_APPLY:
+    case SPARC_GPU_OP_CHEBYSHEV_FILTER:
+    case SPARC_GPU_OP_PROJECT: {
+        int64_t cb = block > 0 ? std::min(block, std::max<int64_t>(ns, 1)) : default_col_block(c, std::max<int64_t>(ns, 1));
+        L->block = cb;
+        L->ldw = round_up_i64(c->nd, 16);
+        L->off_w = off;
+        if (op != SPARC_GPU_OP_HAMILTONIAN_APPLY) off += round_up_i64(L->ldw * cb * 8, A);
+        L->off_d = off;
+        off += round_up_i64((int64_t)std::max(c->n_proj_total, 1) * cb * 8, A);
+        L->off_g = off;
+        if (op == SPARC_GPU_OP_PROJECT) {
+            off += round_up_i64(std::max(gemm_tn_ws_bytes(c, ns, cb, c->nd), gemm_tn_ws_bytes(c, ns, ns, c->nd)), A);
+        }
+        break;
+    }
+    case SPARC_GPU_OP_ROTATE: {
+        int64_t rp = block > 0 ? block : default_row_panel(c, ns);
+        rp = std::min<int64_t>(rp, c->nd);
+        L->block = rp;
+        L->ldw = round_up_i64(rp, 16);
+        L->off_w = off;
+        off += round_up_i64(L->ldw * std::max<int64_t>(ns, 1) * 8, A);
+        break;
+    }
+    default:
+        return SPARC_GPU_INVALID_ARG;
+    }
+    L->total = std::max<int64_t>(off, A);
+    return SPARC_GPU_SUCCESS;
+}
+
+// Out = alpha (H X + shift X) + beta Prev on one column block: fused local pass + nonlocal pair.
+int h_pass(sparc_gpu_ctx *c, const double *X, int64_t ldx, double *Out, int64_t ldo, const double *Prev,
+           int64_t ldp, int64_t ncols, double alpha, double shift, double beta, double *D, cudaStream_t st)
+{
+    int path = c->opt_stencil_path;
+    if (path == 0) path = stencil_tma_supported(c, X, ldx, Out, ldo, Prev, ldp) ? 2 : 1;
+    if (path == 2) {
+        SPARC_TRY(launch_stencil_tma(c, X, ldx, Out, ldo, Prev, ldp, ncols, alpha, shift, beta, st));
+    } else {
+        SPARC_TRY(launch_stencil_generic(c, X, ldx, Out, ldo, Prev, ldp, ncols, alpha, shift, beta, st));
+    }
+    c->stencil_path_last = path;
+    if (c->opt_nonlocal && c->n_atoms > 0 && c->n_proj_total > 0 && c->supp_total > 0) {
+        SPARC_TRY(launch_nl_project(c, X, ldx, ncols, alpha, D, st));
+        SPARC_TRY(launch_nl_pull(c, D, Out, ldo, ncols, st));
+    }
+    return SPARC_GPU_SUCCESS;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *sparc_gpu_version(void) { return "sparc_gpu 0.1.0 (sm_100a)"; }
+
+const char *sparc_gpu_error_string(int code)
+{
+    switch (code) {
+    case SPARC_GPU_SUCCESS: return "success";
+    case SPARC_GPU_INVALID_ARG: return "invalid argument";
+    case SPARC_GPU_UNSUPPORTED: return "unsupported configuration or device";
+    case SPARC_GPU_BAD_BOUNDS: return "filter bounds must satisfy a0 < a < b";
+    case SPARC_GPU_BAD_DESCRIPTOR: return "inconsistent projector descriptor";
+    case SPARC_GPU_WORKSPACE_TOO_SMALL: return "workspace too small";
+    case SPARC_GPU_OUT_OF_MEMORY: return "out of device memory";
+    case SPARC_GPU_CUDA_ERROR: return "CUDA error";
+    default: return "unknown status";
+    }
+}
+
+int sparc_gpu_create(const sparc_gpu_desc *desc, sparc_gpu_ctx **out)
+{
+    if (!desc || !out) return SPARC_GPU_INVALID_ARG;
+    *out = nullptr;
+    SPARC_TRY(validate_desc(desc));
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0) { (void)cudaGetLastError(); return SPARC_GPU_UNSUPPORTED; }
+    if (desc->device < 0 || desc->device >= ndev) return SPARC_GPU_INVALID_ARG;
+    cudaDeviceProp prop;
+    SPARC_CUDA_TRY(cudaGetDeviceProperties(&prop, desc->device));
+    if (prop.major != 10) return SPARC_GPU_UNSUPPORTED;     // sm_100a only, no fallback
+    SPARC_CUDA_TRY(cudaSetDevice(desc->device));
+
+    sparc_gpu_ctx *c = new (std::nothrow) sparc_gpu_ctx();
+    if (!c) return SPARC_GPU_OUT_OF_MEMORY;
+    memset(c, 0, sizeof(*c));
+    c->device = desc->device;
+    c->sm_count = prop.multiProcessorCount;
+    for (int a = 0; a < 3; ++a) { c->n[a] = desc->n[a]; c->h[a] = desc->h[a]; c->bc[a] = desc->bc[a]; }
+    c->radius = desc->fd_order / 2;
+    c->nd = (int64_t)desc->n[0] * desc->n[1] * desc->n[2];
+    c->opt_nonlocal = 1;
+    fd_weights_host(c->radius, c->w);
+    double isum = 0.0;
+    for (int p = 0; p <= SPARC_MAX_RADIUS; ++p) { c->coef.cx[p] = c->coef.cy[p] = c->coef.cz[p] = 0.0; }
+    for (int p = 1; p <= c->radius; ++p) {
+        c->coef.cx[p] = -0.5 * c->w[p] / (c->h[0] * c->h[0]);
+        c->coef.cy[p] = -0.5 * c->w[p] / (c->h[1] * c->h[1]);
+        c->coef.cz[p] = -0.5 * c->w[p] / (c->h[2] * c->h[2]);
+    }
+    for (int a = 0; a < 3; ++a) isum += 1.0 / (c->h[a] * c->h[a]);
+    c->coef.c0 = -0.5 * c->w[0] * isum;
+
+    // resolve cuTensorMapEncodeTiled without linking libcuda
+    {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            c->fn_encode_tiled = fn;
+        else
+            (void)cudaGetLastError();
+    }
+
+    int st = SPARC_GPU_SUCCESS;
+    do {
+        // local potential
+        if ((st = (cudaMalloc((void **)&c->d_veff, (size_t)c->nd * 8) == cudaSuccess) ? 0 : SPARC_GPU_OUT_OF_MEMORY)) break;
+        if (desc->veff) {
+            if (cudaMemcpy(c->d_veff, desc->veff, (size_t)c->nd * 8, cudaMemcpyHostToDevice) != cudaSuccess) { st = SPARC_GPU_CUDA_ERROR; break; }
+        } else if (cudaMemset(c->d_veff, 0, (size_t)c->nd * 8) != cudaSuccess) { st = SPARC_GPU_CUDA_ERROR; break; }
+
+        c->n_atoms = desc->n_atoms;
+        if (c->n_atoms == 0) break;
+        const int na = c->n_atoms;
+        c->supp_total = desc->supp_ptr[na];
+        std::vector<int32_t> pofs(na + 1, 0);
+        for (int J = 0; J < na; ++J) {
+            pofs[J + 1] = pofs[J] + desc->n_proj[J];
+            c->max_proj = std::max<int32_t>(c->max_proj, desc->n_proj[J]);
+        }
+        c->n_proj_total = pofs[na];
+        if ((st = upload(&c->d_supp_ptr, desc->supp_ptr, (size_t)na + 1))) break;
+        if ((st = upload(&c->d_supp_idx, desc->supp_idx, (size_t)c->supp_total))) break;
+        if ((st = upload(&c->d_n_proj, desc->n_proj, (size_t)na))) break;
+        if ((st = upload(&c->d_proj_ofs, pofs.data(), (size_t)na + 1))) break;
+        if ((st = upload(&c->d_chi_ptr, desc->chi_ptr, (size_t)na + 1))) break;
+        if ((st = upload(&c->d_chi, desc->chi, (size_t)desc->chi_ptr[na]))) break;
+        if ((st = upload(&c->d_gamma, desc->gamma, (size_t)c->n_proj_total))) break;
+
+        // inverse map point -> list of (atom, row): counting sort by grid index
+        std::vector<int64_t> cnt((size_t)c->nd + 1, 0);
+        for (int64_t t = 0; t < c->supp_total; ++t) cnt[(size_t)desc->supp_idx[t] + 1]++;
+        std::vector<int32_t> cov_idx;
+        std::vector<int64_t> cov_ptr;
+        std::vector<int64_t> slot((size_t)c->nd, -1);
+        cov_ptr.push_back(0);
+        for (int64_t i = 0; i < c->nd; ++i) {
+            if (cnt[(size_t)i + 1] > 0) {
+                slot[(size_t)i] = cov_ptr.back();
+                cov_idx.push_back((int32_t)i);
+                cov_ptr.push_back(cov_ptr.back() + cnt[(size_t)i + 1]);
+            }
+        }
+        c->n_covered = (int64_t)cov_idx.size();
+        std::vector<CoverEntry> ent((size_t)c->supp_total);
+        for (int J = 0; J < na; ++J) {
+            const int64_t s0 = desc->supp_ptr[J], nJ = desc->supp_ptr[J + 1] - s0;
+            for (int64_t t = 0; t < nJ; ++t) {
+                const int32_t i = desc->supp_idx[s0 + t];
+                CoverEntry e;
+                e.chi_off = desc->chi_ptr[J] + t;
+                e.n_j = (int32_t)nJ;
+                e.pofs_p = (pofs[J] << 8) | desc->n_proj[J];
+                ent[(size_t)slot[(size_t)i]++] = e;      // atoms in ascending J order per point: deterministic
+            }
+        }
+        if ((st = upload(&c->d_cov_idx, cov_idx.data(), cov_idx.size()))) break;
+        if ((st = upload(&c->d_cov_ptr, cov_ptr.data(), cov_ptr.size()))) break;
+        if ((st = upload(&c->d_cov_ent, ent.data(), ent.size()))) break;
+    } while (0);
+    if (st != SPARC_GPU_SUCCESS) { (void)cudaGetLastError(); free_tables(c); delete c; return st; }
+    *out = c;
+    return SPARC_GPU_SUCCESS;
+}
+
+int sparc_gpu_destroy(sparc_gpu_ctx *ctx)
+{
+    if (!ctx) return SPARC_GPU_INVALID_ARG;
+    cudaSetDevice(ctx->device);
+    free_tables(ctx);
+    delete ctx;
+    return SPARC_GPU_SUCCESS;
+}
+
+int sparc_gpu_set_veff(sparc_gpu_ctx *ctx, const double *veff_dev, void *stream)
+{
+    if (!ctx || !veff_dev) return SPARC_GPU_INVALID_ARG;
+    SPARC_CUDA_TRY(cudaMemcpyAsync(ctx->d_veff, veff_dev, (size_t)ctx->nd * 8, cudaMemcpyDeviceToDevice,
+                                   (cudaStream_t)stream));
+    return SPARC_GPU_SUCCESS;
+}
+
+int sparc_gpu_set_option(sparc_gpu_ctx *ctx, const char *key, int64_t value)
+{
+    if (!ctx || !key) return SPARC_GPU_INVALID_ARG;
+    if (!strcmp(key, "stencil_path")) { if (value < 0 || value > 2) return SPARC_GPU_INVALID_ARG; ctx->opt_stencil_path = (int)value; return 0; }
+    if (!strcmp(key, "nonlocal")) { ctx->opt_nonlocal = value ? 1 : 0; return 0; }
+    if (!strcmp(key, "gemm_path")) { if (value < 0 || value > 2) return SPARC_GPU_INVALID_ARG; ctx->opt_gemm_path = (int)value; return 0; }
+    return SPARC_GPU_INVALID_ARG;
+}
+
+int sparc_gpu_get_info(const sparc_gpu_ctx *ctx, const char *key, int64_t *value)
+{
+    if (!ctx || !key || !value) return SPARC_GPU_INVALID_ARG;
+    if (!strcmp(key, "kernel_launches")) { *value = ctx->kernel_launches; return 0; }
+    if (!strcmp(key, "nd")) { *value = ctx->nd; return 0; }
+    if (!strcmp(key, "n_proj_total")) { *value = ctx->n_proj_total; return 0; }
+    if (!strcmp(key, "covered_points")) { *value = ctx->n_covered; return 0; }
+    if (!strcmp(key, "stencil_path_last")) { *value = ctx->stencil_path_last; return 0; }
+    if (!strcmp(key, "sm_count")) { *value = ctx->sm_count; return 0; }
+    return SPARC_GPU_INVALID_ARG;
+}
+
+int sparc_gpu_workspace_bytes(const sparc_gpu_ctx *ctx, int op, int64_t ns, int64_t block, int64_t *bytes)
+{
+    if (!ctx || !bytes) return SPARC_GPU_INVALID_ARG;
+    WsLayout L;
+    SPARC_TRY(ws_layout(ctx, op, ns, block, &L));
+    *bytes = L.total;
+    return SPARC_GPU_SUCCESS;
+}
+
+int sparc_gpu_hamiltonian_apply(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double *Y, int64_t ldy,
+                                int64_t ncols, void *ws, void *stream)
+{
+    if (!ctx || ncols < 0) return SPARC_GPU_INVALID_ARG;
+    if (ncols == 0) return SPARC_GPU_SUCCESS;
+    if (!X || !Y || !ws || ldx < ctx->nd || ldy < ctx->nd) return SPARC_GPU_INVALID_ARG;
+    SPARC_CUDA_TRY(cudaSetDevice(ctx->device));
+    WsLayout L;
+    SPARC_TRY(ws_layout(ctx, SPARC_GPU_OP_HAMILTONIAN_APPLY, ncols, 0, &L));
+    double *D = (double *)((char *)ws + L.off_d);
+    for (int64_t j0 = 0; j0 < ncols; j0 += L.block) {
+        const int64_t nb = std::min(L.block, ncols - j0);
+        SPARC_TRY(h_pass(ctx, X + j0 * ldx, ldx, Y + j0 * ldy, ldy, nullptr, 0, nb, 1.0, 0.0, 0.0, D,
+                         (cudaStream_t)stream));
+    }
+    return SPARC_GPU_SUCCESS;
+}
+
+int sparc_gpu_chebyshev_filter(sparc_gpu_ctx *ctx, double *Psi, int64_t ld, int64_t ns, int degree, double a,
+                               double b, double a0, int64_t col_block, void *ws, void *stream)
+{
+    if (!ctx || ns < 0 || degree < 0) return SPARC_GPU_INVALID_ARG;
+    if (!(a0 < a && a < b)) return SPARC_GPU_BAD_BOUNDS;
+    if (ns == 0 || degree == 0) return SPARC_GPU_SUCCESS;
+    if (!Psi || !ws || ld < ctx->nd) return SPARC_GPU_INVALID_ARG;
+    SPARC_CUDA_TRY(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    WsLayout L;
+    SPARC_TRY(ws_layout(ctx, SPARC_GPU_OP_CHEBYSHEV_FILTER, ns, col_block, &L));
+    double *W = (double *)((char *)ws + L.off_w);
+    double *D = (double *)((char *)ws + L.off_d);
+    const double e = 0.5 * (b - a), c = 0.5 * (b + a);
+    const double sigma1 = e / (a0 - c), tau = 2.0 / sigma1;
+    for (int64_t j0 = 0; j0 < ns; j0 += L.block) {
+        const int64_t nb = std::min(L.block, ns - j0);
+        double *bufA = Psi + j0 * ld;     // holds Y_{k-1} (k odd) / Y_k (k even)
+        double *cur = bufA, *oth = W;
+        int64_t ldc = ld, ldo = L.ldw;
+        // k = 1:  oth = (sigma1/e)(H cur - c cur)
+        SPARC_TRY(h_pass(ctx, cur, ldc, oth, ldo, nullptr, 0, nb, sigma1 / e, -c, 0.0, D, st));
+        double sigma = sigma1;
+        std::swap(cur, oth); std::swap(ldc, ldo);
+        for (int k = 2; k <= degree; ++k) {
+            const double sigma2 = 1.0 / (tau - sigma);
+            // oth (= Y_{k-2}) <- (2 sigma2/e)(H cur - c cur) - sigma sigma2 * oth
+            SPARC_TRY(h_pass(ctx, cur, ldc, oth, ldo, oth, ldo, nb, 2.0 * sigma2 / e, -c, -(sigma * sigma2), D, st));
+            sigma = sigma2;
+            std::swap(cur, oth); std::swap(ldc, ldo);
+        }
+        if (cur != bufA) SPARC_TRY(launch_copy_2d(ctx, bufA, ld, cur, ldc, ctx->nd, nb, st));
+    }
+    return SPARC_GPU_SUCCESS;
+}
+
+int sparc_gpu_project(sparc_gpu_ctx *ctx, const double *Psi, int64_t ld, int64_t ns, double *Hs, double *Ms,
+                      int64_t col_block, void *ws, void *stream)
+{
+    if (!ctx || ns < 0) return SPARC_GPU_INVALID_ARG;
+    if (ns == 0) return SPARC_GPU_SUCCESS;
+    if (!Psi || !Hs || !Ms || !ws || ld < ctx->nd) return SPARC_GPU_INVALID_ARG;
+    SPARC_CUDA_TRY(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    WsLayout L;
+    SPARC_TRY(ws_layout(ctx, SPARC_GPU_OP_PROJECT, ns, col_block, &L));
+    double *Y = (double *)((char *)ws + L.off_w);
+    double *D = (double *)((char *)ws + L.off_d);
+    void *G = (char *)ws + L.off_g;
+    for (int64_t j0 = 0; j0 < ns; j0 += L.block) {
+        const int64_t nb = std::min(L.block, ns - j0);
+        SPARC_TRY(h_pass(ctx, Psi + j0 * ld, ld, Y, L.ldw, nullptr, 0, nb, 1.0, 0.0, 0.0, D, st));
+        // Hs[:, j0:j0+nb] = Psi^T Y_block
+        SPARC_TRY(launch_gemm_tn(ctx, Psi, ld, Y, L.ldw, Hs + j0 * ns, ns, ns, nb, ctx->nd, G, st));
+    }
+    SPARC_TRY(launch_gemm_tn(ctx, Psi, ld, Psi, ld, Ms, ns, ns, ns, ctx->nd, G, st));
+    return SPARC_GPU_SUCCESS;
+}
+
+int sparc_gpu_rotate(sparc_gpu_ctx *ctx, double *Psi, int64_t ld, int64_t ns, const double *Q, int64_t row_panel,
+                     void *ws, void *stream)
+{
+    if (!ctx || ns < 0) return SPARC_GPU_INVALID_ARG;
+    if (ns == 0) return SPARC_GPU_SUCCESS;
+    if (!Psi || !Q || !ws || ld < ctx->nd) return SPARC_GPU_INVALID_ARG;
+    SPARC_CUDA_TRY(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    WsLayout L;
+    SPARC_TRY(ws_layout(ctx, SPARC_GPU_OP_ROTATE, ns, row_panel, &L));
+    double *T = (double *)((char *)ws + L.off_w);
+    for (int64_t r0 = 0; r0 < ctx->nd; r0 += L.block) {
+        const int64_t nr = std::min(L.block, ctx->nd - r0);
+        SPARC_TRY(launch_gemm_nn(ctx, Psi + r0, ld, Q, ns, T, L.ldw, nr, ns, ns, st));
+        SPARC_TRY(launch_copy_2d(ctx, Psi + r0, ld, T, L.ldw, nr, ns, st));
+    }
+    return SPARC_GPU_SUCCESS;
+}
+
+}  // extern "C"

@@ -1,0 +1,269 @@
+// gemm.cu -- FP64 tensor-core (DMMA m8n8k4) tiled GEMMs for the subspace steps:
+//   TN:  C = A^T B  with the contraction over the N_d grid rows   (Hs = Psi^T Y, Ms = Psi^T Psi)
+//   NN:  C = A B    row panel of Psi times Q                      (X = X~ Z~)
+// On sm_100a every PTX f64 mma.sync shape lowers to DMMA.8x8x4, so m8n8k4 is used directly.  Operands are
+// staged global -> shared with cp.async (3 stages), fragments are read with conflict-free LDS.64 (row pitch
+// == 4 mod 16 doubles).  tcgen05/TMEM have no f64 kind and do not apply here.
+// Small-output TN products (N_s = 32, 256) are split over K across the chip and reduced in a fixed order
+// (deterministic).
+#include <algorithm>
+
+#include "internal.h"
+
+namespace {
+
+constexpr int BM = 128, BN = 128, BK = 16, STAGES = 3;
+constexpr int PITCH_K = BK + 4;     // rows of BK doubles (k contiguous)
+constexpr int PITCH_M = BM + 4;     // rows of BM doubles (m contiguous)
+constexpr int GEMM_THREADS = 256;
+
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem, int src_bytes)
+{
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(src_bytes));
+}
+__device__ __forceinline__ void cp_async8(void *smem, const void *gmem, int src_bytes)
+{
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(s), "l"(gmem), "r"(src_bytes));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+__device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
+
+constexpr size_t smem_bytes(bool a_mmajor)
+{
+    return (size_t)STAGES * ((a_mmajor ? BK * PITCH_M : BM * PITCH_K) + BN * PITCH_K) * sizeof(double);
+}
+
+// Load a tile whose contiguous global direction is "inner" (length INNER doubles per row, ROWS rows).
+// Global element (inner i, row r) lives at g[i + r*ld]; rows beyond `rows_valid` and inner beyond
+// `inner_valid` are zero-filled.  Shared layout: s[r*PITCH + i].
+template <int ROWS, int INNER, int PITCH, bool VEC16>
+__device__ __forceinline__ void load_tile(double *s, const double *g, int64_t ld, int64_t rows_valid,
+                                          int64_t inner_valid, int tid)
+{
+    if (VEC16) {
+        constexpr int CH = INNER / 2;
+        for (int c = tid; c < ROWS * CH; c += GEMM_THREADS) {
+            const int r = c / CH, i = (c % CH) * 2;
+            int bytes = 0;
+            if (r < rows_valid) bytes = (i + 1 < inner_valid) ? 16 : ((i < inner_valid) ? 8 : 0);
+            const double *src = bytes ? g + i + (int64_t)r * ld : g;
+            cp_async16(s + r * PITCH + i, src, bytes);
+        }
+    } else {
+        for (int c = tid; c < ROWS * INNER; c += GEMM_THREADS) {
+            const int r = c / INNER, i = c % INNER;
+            const int bytes = (r < rows_valid && i < inner_valid) ? 8 : 0;
+            const double *src = bytes ? g + i + (int64_t)r * ld : g;
+            cp_async8(s + r * PITCH + i, src, bytes);
+        }
+    }
+}
+
+// A_MMAJOR = false: A is K x M col-major (A[k + m*lda]) -> C = A^T B           (TN)
+// A_MMAJOR = true : A is M x K col-major (A[m + k*lda]) -> C = A B             (NN)
+// B is always K x N col-major (B[k + n*ldb]).  C is M x N col-major; with splits > 1, blockIdx.z writes its
+// partial product to Cpart + z*M*N (ld = M).
+template <bool A_MMAJOR, bool VEC16>
+__global__ void __launch_bounds__(GEMM_THREADS, 1)
+gemm_dmma_kernel(const double *__restrict__ A, int64_t lda, const double *__restrict__ B, int64_t ldb, double *C,
+                 int64_t ldc, int64_t M, int64_t N, int64_t K, int64_t k_chunk, int tiles_m)
+{
+    extern __shared__ __align__(16) double smem[];
+    constexpr int A_STAGE = A_MMAJOR ? BK * PITCH_M : BM * PITCH_K;
+    constexpr int B_STAGE = BN * PITCH_K;
+    double *As = smem;
+    double *Bs = smem + STAGES * A_STAGE;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wm = warp >> 2, wn = warp & 3;          // 2 x 4 warps, warp tile 64 x 32
+    const int tile_m = blockIdx.x % tiles_m, tile_n = blockIdx.x / tiles_m;
+    const int64_t m0 = (int64_t)tile_m * BM, n0 = (int64_t)tile_n * BN;
+    const int64_t k_begin = (int64_t)blockIdx.z * k_chunk;
+    const int64_t k_end = (k_begin + k_chunk < K) ? k_begin + k_chunk : K;
+    if (gridDim.z > 1) { C += (int64_t)blockIdx.z * M * N; ldc = M; }
+    const int nkt = (k_end > k_begin) ? (int)((k_end - k_begin + BK - 1) / BK) : 0;
+
+    double acc[8][4][2];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    auto issue = [&](int kt) {
+        const int s = kt % STAGES;
+        const int64_t k0 = k_begin + (int64_t)kt * BK;
+        const int64_t kv = k_end - k0;      // valid k in this tile (may exceed BK)
+        if (A_MMAJOR)
+            load_tile<BK, BM, PITCH_M, VEC16>(As + s * A_STAGE, A + m0 + k0 * lda, lda, kv, M - m0, tid);
+        else
+            load_tile<BM, BK, PITCH_K, VEC16>(As + s * A_STAGE, A + k0 + m0 * lda, lda, M - m0, kv, tid);
+        load_tile<BN, BK, PITCH_K, VEC16>(Bs + s * B_STAGE, B + k0 + n0 * ldb, ldb, N - n0, kv, tid);
+    };
+
+#pragma unroll
+    for (int s = 0; s < STAGES - 1; ++s) {
+        if (s < nkt) issue(s);
+        cp_async_commit();
+    }
+    const int lr = lane >> 2, lk = lane & 3;
+    for (int kt = 0; kt < nkt; ++kt) {
+        cp_async_wait<STAGES - 2>();
+        __syncthreads();
+        if (kt + STAGES - 1 < nkt) issue(kt + STAGES - 1);
+        cp_async_commit();
+        const double *as = As + (kt % STAGES) * A_STAGE;
+        const double *bs = Bs + (kt % STAGES) * B_STAGE;
+#pragma unroll
+        for (int kk = 0; kk < BK; kk += 4) {
+            double a[8], b[4];
+#pragma unroll
+            for (int mi = 0; mi < 8; ++mi) {
+                const int m = wm * 64 + mi * 8 + lr;
+                a[mi] = A_MMAJOR ? as[(kk + lk) * PITCH_M + m] : as[m * PITCH_K + kk + lk];
+            }
+#pragma unroll
+            for (int ni = 0; ni < 4; ++ni) b[ni] = bs[(wn * 32 + ni * 8 + lr) * PITCH_K + kk + lk];
+#pragma unroll
+            for (int mi = 0; mi < 8; ++mi)
+#pragma unroll
+                for (int ni = 0; ni < 4; ++ni) dmma884(acc[mi][ni][0], acc[mi][ni][1], a[mi], b[ni]);
+        }
+    }
+    cp_async_wait<0>();
+
+#pragma unroll
+    for (int mi = 0; mi < 8; ++mi) {
+        const int64_t row = m0 + wm * 64 + mi * 8 + lr;
+        if (row >= M) continue;
+#pragma unroll
+        for (int ni = 0; ni < 4; ++ni) {
+            const int64_t col = n0 + wn * 32 + ni * 8 + 2 * lk;
+            if (col < N) C[row + col * ldc] = acc[mi][ni][0];
+            if (col + 1 < N) C[row + (col + 1) * ldc] = acc[mi][ni][1];
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256)
+splitk_reduce_kernel(const double *__restrict__ part, int splits, int64_t M, int64_t N, double *C, int64_t ldc)
+{
+    const int64_t total = M * N;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
+        double s = 0.0;
+        for (int z = 0; z < splits; ++z) s += part[(int64_t)z * total + e];     // fixed order: deterministic
+        C[(e % M) + (e / M) * ldc] = s;
+    }
+}
+
+// Reference-shaped simple kernel (option gemm_path = 1): one thread per output element, plain FMA loop.
+template <bool A_MMAJOR>
+__global__ void __launch_bounds__(256)
+gemm_simple_kernel(const double *__restrict__ A, int64_t lda, const double *__restrict__ B, int64_t ldb, double *C,
+                   int64_t ldc, int64_t M, int64_t N, int64_t K)
+{
+    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= M * N) return;
+    const int64_t m = e % M, n = e / M;
+    double s = 0.0;
+    for (int64_t k = 0; k < K; ++k) s = fma(A_MMAJOR ? A[m + k * lda] : A[k + m * lda], B[k + n * ldb], s);
+    C[m + n * ldc] = s;
+}
+
+struct SplitPlan { int splits; int64_t k_chunk; };
+
+SplitPlan plan_tn(const sparc_gpu_ctx *ctx, int64_t M, int64_t N, int64_t K)
+{
+    const int64_t tiles = ((M + BM - 1) / BM) * ((N + BN - 1) / BN);
+    int64_t splits = 1;
+    if (tiles < (int64_t)ctx->sm_count) {
+        splits = (2 * (int64_t)ctx->sm_count + tiles - 1) / tiles;
+        const int64_t max_splits = std::max<int64_t>(1, K / (8 * BK));
+        splits = std::max<int64_t>(1, std::min(splits, max_splits));
+    }
+    int64_t chunk = (K + splits - 1) / splits;
+    chunk = round_up_i64(std::max<int64_t>(chunk, 1), BK);
+    splits = (K + chunk - 1) / chunk;
+    if (splits < 1) splits = 1;
+    return {(int)splits, chunk};
+}
+
+bool aligned16(const void *p) { return ((uintptr_t)p & 15) == 0; }
+
+template <bool A_MMAJOR>
+int launch_dmma(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const double *B, int64_t ldb, double *C, int64_t ldc,
+                int64_t M, int64_t N, int64_t K, SplitPlan plan, cudaStream_t st)
+{
+    const int tiles_m = (int)((M + BM - 1) / BM), tiles_n = (int)((N + BN - 1) / BN);
+    dim3 grid((unsigned)(tiles_m * tiles_n), 1, (unsigned)plan.splits);
+    const bool vec = aligned16(A) && aligned16(B) && (lda % 2 == 0) && (ldb % 2 == 0);
+    const size_t smem = smem_bytes(A_MMAJOR);
+    if (vec) {
+        auto kern = gemm_dmma_kernel<A_MMAJOR, true>;
+        SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kern<<<grid, GEMM_THREADS, smem, st>>>(A, lda, B, ldb, C, ldc, M, N, K, plan.k_chunk, tiles_m);
+    } else {
+        auto kern = gemm_dmma_kernel<A_MMAJOR, false>;
+        SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kern<<<grid, GEMM_THREADS, smem, st>>>(A, lda, B, ldb, C, ldc, M, N, K, plan.k_chunk, tiles_m);
+    }
+    ctx->kernel_launches++;
+    SPARC_CUDA_TRY(cudaGetLastError());
+    return SPARC_GPU_SUCCESS;
+}
+
+}  // namespace
+
+int64_t gemm_tn_ws_bytes(const sparc_gpu_ctx *ctx, int64_t M, int64_t N, int64_t K)
+{
+    SplitPlan p = plan_tn(ctx, M, N, K);
+    return p.splits > 1 ? (int64_t)p.splits * M * N * 8 : 0;
+}
+
+int launch_gemm_tn(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const double *B, int64_t ldb, double *C,
+                   int64_t ldc, int64_t M, int64_t N, int64_t K, void *ws, cudaStream_t st)
+{
+    if (M <= 0 || N <= 0) return SPARC_GPU_SUCCESS;
+    if (ctx->opt_gemm_path == 1) {
+        const int64_t blocks = (M * N + 255) / 256;
+        gemm_simple_kernel<false><<<(unsigned)blocks, 256, 0, st>>>(A, lda, B, ldb, C, ldc, M, N, K);
+        ctx->kernel_launches++;
+        SPARC_CUDA_TRY(cudaGetLastError());
+        return SPARC_GPU_SUCCESS;
+    }
+    SplitPlan plan = plan_tn(ctx, M, N, K);
+    if (plan.splits > 1) {
+        double *part = (double *)ws;
+        SPARC_TRY(launch_dmma<false>(ctx, A, lda, B, ldb, part, M, M, N, K, plan, st));
+        int64_t blocks = std::min<int64_t>((M * N + 255) / 256, (int64_t)ctx->sm_count * 8);
+        splitk_reduce_kernel<<<(unsigned)blocks, 256, 0, st>>>(part, plan.splits, M, N, C, ldc);
+        ctx->kernel_launches++;
+        SPARC_CUDA_TRY(cudaGetLastError());
+        return SPARC_GPU_SUCCESS;
+    }
+    return launch_dmma<false>(ctx, A, lda, B, ldb, C, ldc, M, N, K, plan, st);
+}
+
+int launch_gemm_nn(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const double *B, int64_t ldb, double *C,
+                   int64_t ldc, int64_t M, int64_t N, int64_t K, cudaStream_t st)
+{
+    if (M <= 0 || N <= 0) return SPARC_GPU_SUCCESS;
+    if (ctx->opt_gemm_path == 1) {
+        const int64_t blocks = (M * N + 255) / 256;
+        gemm_simple_kernel<true><<<(unsigned)blocks, 256, 0, st>>>(A, lda, B, ldb, C, ldc, M, N, K);
+        ctx->kernel_launches++;
+        SPARC_CUDA_TRY(cudaGetLastError());
+        return SPARC_GPU_SUCCESS;
+    }
+    SplitPlan plan{1, round_up_i64(std::max<int64_t>(K, 1), BK)};
+    return launch_dmma<true>(ctx, A, lda, B, ldb, C, ldc, M, N, K, plan, st);
+}

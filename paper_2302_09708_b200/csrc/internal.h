@@ -1,0 +1,115 @@
+// internal.h -- shared declarations of the sparc_gpu CUDA library (product code; not used by oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/sparc_gpu.h"
+
+#define SPARC_MAX_RADIUS 6
+#define SPARC_MAX_PROJ 16
+
+// Coefficients of one fused stencil pass.  With H_loc = -1/2 L + Veff the kernel computes
+//   Out = alpha * (H_loc X + shift * X) + beta * Prev
+// cx/cy/cz[p] = -1/2 * w_p / h_axis^2 (p = 1..radius), c0 = -1/2 * w_0 * sum_axis 1/h_axis^2.
+struct StencilCoef {
+    double cx[SPARC_MAX_RADIUS + 1];
+    double cy[SPARC_MAX_RADIUS + 1];
+    double cz[SPARC_MAX_RADIUS + 1];
+    double c0;
+};
+
+// One entry of the point -> (atom, support row) inverse map used by the nonlocal pull kernel.
+struct CoverEntry {
+    int64_t chi_off;   // offset (doubles) of chi_J[t, 0]
+    int32_t n_j;       // stride between projector columns of chi_J
+    int32_t pofs_p;    // (offset of atom J's first projector in D) << 8 | P_J
+};
+
+struct sparc_gpu_ctx {
+    int device;
+    int sm_count;
+    int32_t n[3];
+    double h[3];
+    int32_t bc[3];
+    int32_t radius;
+    int64_t nd;
+    StencilCoef coef;          // alpha = 1 coefficients (host copy)
+    double w[SPARC_MAX_RADIUS + 1];
+    // nonlocal tables (device)
+    int32_t n_atoms;
+    int32_t n_proj_total;
+    int32_t max_proj;
+    int64_t supp_total;
+    int64_t *d_supp_ptr;       // [n_atoms+1]
+    int32_t *d_supp_idx;       // [supp_total]
+    int32_t *d_n_proj;         // [n_atoms]
+    int32_t *d_proj_ofs;       // [n_atoms+1] prefix sum of n_proj
+    int64_t *d_chi_ptr;        // [n_atoms+1]
+    double *d_chi;
+    double *d_gamma;           // [n_proj_total]
+    // inverse (pull) map
+    int64_t n_covered;
+    int32_t *d_cov_idx;        // [n_covered] grid index of each covered point (ascending)
+    int64_t *d_cov_ptr;        // [n_covered+1] offsets into d_cov_ent
+    CoverEntry *d_cov_ent;     // [supp_total]
+    // local potential
+    double *d_veff;            // [nd]
+    // options
+    int opt_stencil_path;      // 0 auto, 1 generic, 2 TMA
+    int opt_nonlocal;          // 1 on
+    int opt_gemm_path;         // 0 auto, 1 simple, 2 DMMA
+    // counters
+    mutable int64_t kernel_launches;
+    int stencil_path_last;
+    // driver entry point for tensor-map encoding (resolved at create; NULL if unavailable)
+    void *fn_encode_tiled;
+};
+
+#define SPARC_CUDA_TRY(expr)                                         \
+    do {                                                             \
+        cudaError_t _e = (expr);                                     \
+        if (_e != cudaSuccess) {                                     \
+            (void)cudaGetLastError();                                \
+            return (_e == cudaErrorMemoryAllocation) ? SPARC_GPU_OUT_OF_MEMORY : SPARC_GPU_CUDA_ERROR; \
+        }                                                            \
+    } while (0)
+
+#define SPARC_TRY(expr)                    \
+    do {                                   \
+        int _s = (expr);                   \
+        if (_s != SPARC_GPU_SUCCESS) return _s; \
+    } while (0)
+
+static inline int64_t round_up_i64(int64_t v, int64_t m) { return (v + m - 1) / m * m; }
+
+// ---- kernel launchers (each returns a sparc_gpu_status and bumps ctx->kernel_launches) ----------
+
+// Out = alpha * (H_loc X + shift X) + beta * Prev   (Prev may be NULL when beta == 0; Prev may alias Out)
+int launch_stencil_generic(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double *Out, int64_t ldo,
+                           const double *Prev, int64_t ldp, int64_t ncols, double alpha, double shift,
+                           double beta, cudaStream_t st);
+// same contract; returns SPARC_GPU_UNSUPPORTED if the shape does not meet the TMA kernel's preconditions
+int launch_stencil_tma(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double *Out, int64_t ldo,
+                       const double *Prev, int64_t ldp, int64_t ncols, double alpha, double shift,
+                       double beta, cudaStream_t st);
+bool stencil_tma_supported(const sparc_gpu_ctx *ctx, const double *X, int64_t ldx, const double *Out,
+                           int64_t ldo, const double *Prev, int64_t ldp);
+
+// D[q, col] = scale * gamma[q] * sum_t chi[t, q] X[idx[t], col]     (D: n_proj_total x ncols, ld = n_proj_total)
+int launch_nl_project(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, int64_t ncols, double scale,
+                      double *D, cudaStream_t st);
+// Out[i, col] += sum_{(J,t) covering i} sum_q chi_J[t, q] D[ofs_J + q, col]
+int launch_nl_pull(sparc_gpu_ctx *ctx, const double *D, double *Out, int64_t ldo, int64_t ncols,
+                   cudaStream_t st);
+
+// C (M x N, col-major, ldc) = A^T B, A: K x M (lda), B: K x N (ldb), contraction over K rows.
+// ws: split-K partials (gemm_tn_ws_bytes).  symmetric_out: A == B, fill lower from upper.
+int64_t gemm_tn_ws_bytes(const sparc_gpu_ctx *ctx, int64_t M, int64_t N, int64_t K);
+int launch_gemm_tn(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const double *B, int64_t ldb,
+                   double *C, int64_t ldc, int64_t M, int64_t N, int64_t K, void *ws, cudaStream_t st);
+// C (M x N, ldc) = A B, A: M x K col-major (lda), B: K x N col-major (ldb)
+int launch_gemm_nn(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const double *B, int64_t ldb,
+                   double *C, int64_t ldc, int64_t M, int64_t N, int64_t K, cudaStream_t st);
+// dst (rows x cols, ldd) = src (rows x cols, lds)
+int launch_copy_2d(sparc_gpu_ctx *ctx, double *dst, int64_t ldd, const double *src, int64_t lds,
+                   int64_t rows, int64_t cols, cudaStream_t st);

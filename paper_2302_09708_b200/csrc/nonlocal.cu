@@ -1,0 +1,142 @@
+// nonlocal.cu -- Kleinman-Bylander nonlocal term  V_nl X = sum_J S_J^T chi_J diag(gamma_J) chi_J^T S_J X
+// ("nonlocal projectors for each atom, stored as a dense matrix, are applied on the
+// appropriate components of X").  Two kernels:
+//   nl_project : D_J = scale * diag(gamma_J) chi_J^T X[idx_J, cols]     warp-cooperative gather + small GEMM
+//   nl_pull    : Out[i, col] += sum_{(J,t) covers i} chi_J[t,:] . D_J[:, col]
+// The second is the scatter written in pull (gather) form through the point -> (atom,row) inverse map
+// built at create: conflict-free without atomics and bitwise reproducible (R15).
+#include <algorithm>
+
+#include "internal.h"
+
+namespace {
+
+constexpr int NLP_WARPS = 8;      // warps per CTA in nl_project
+constexpr int NLP_COLS = 4;       // columns per warp
+
+// grid: (n_atoms, ceil(ncols / (NLP_WARPS*NLP_COLS))).  Lanes stride over the support rows t; each lane keeps
+// PMAX x NLP_COLS partial sums; a shuffle tree reduces them; lane 0 scales by gamma and writes D.
+template <int PMAX>
+__global__ void __launch_bounds__(NLP_WARPS * 32)
+nl_project_kernel(const int64_t *__restrict__ supp_ptr, const int32_t *__restrict__ supp_idx,
+                  const int32_t *__restrict__ n_proj, const int32_t *__restrict__ proj_ofs,
+                  const int64_t *__restrict__ chi_ptr, const double *__restrict__ chi,
+                  const double *__restrict__ gamma, const double *__restrict__ X, int64_t ldx, int64_t ncols,
+                  double scale, double *__restrict__ D, int ldD)
+{
+    const int J = blockIdx.x;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t col0 = ((int64_t)blockIdx.y * NLP_WARPS + warp) * NLP_COLS;
+    if (col0 >= ncols) return;
+    const int P = n_proj[J];
+    if (P == 0) return;
+    const int64_t s0 = supp_ptr[J];
+    const int nJ = (int)(supp_ptr[J + 1] - s0);
+    const int32_t *idx = supp_idx + s0;
+    const double *ch = chi + chi_ptr[J];
+    const double *xc[NLP_COLS];
+#pragma unroll
+    for (int c = 0; c < NLP_COLS; ++c) xc[c] = X + (col0 + c < ncols ? col0 + c : col0) * ldx;
+
+    double acc[PMAX][NLP_COLS];
+#pragma unroll
+    for (int q = 0; q < PMAX; ++q)
+#pragma unroll
+        for (int c = 0; c < NLP_COLS; ++c) acc[q][c] = 0.0;
+
+    for (int t = lane; t < nJ; t += 32) {
+        const int i = idx[t];
+        double g[NLP_COLS];
+#pragma unroll
+        for (int c = 0; c < NLP_COLS; ++c) g[c] = xc[c][i];
+#pragma unroll
+        for (int q = 0; q < PMAX; ++q) {
+            if (q < P) {
+                const double cv = ch[t + (int64_t)q * nJ];
+#pragma unroll
+                for (int c = 0; c < NLP_COLS; ++c) acc[q][c] = fma(cv, g[c], acc[q][c]);
+            }
+        }
+    }
+    const int po = proj_ofs[J];
+#pragma unroll
+    for (int q = 0; q < PMAX; ++q) {
+        if (q < P) {
+#pragma unroll
+            for (int c = 0; c < NLP_COLS; ++c) {
+                double v = acc[q][c];
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                if (lane == 0 && col0 + c < ncols) D[(int64_t)(po + q) + (col0 + c) * (int64_t)ldD] = scale * gamma[po + q] * v;
+            }
+        }
+    }
+}
+
+// grid: (ceil(n_covered/128), column chunks).  One thread per covered point, looping over the columns of
+// its chunk: consecutive covered points are mostly consecutive grid indices -> coalesced read-modify-write.
+__global__ void __launch_bounds__(128)
+nl_pull_kernel(const int32_t *__restrict__ cov_idx, const int64_t *__restrict__ cov_ptr,
+               const CoverEntry *__restrict__ ent, const double *__restrict__ chi, const double *__restrict__ D,
+               int ldD, double *Out, int64_t ldo, int64_t n_covered, int64_t ncols, int cols_per_block)
+{
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_covered) return;
+    const int i = cov_idx[k];
+    const int64_t e0 = cov_ptr[k], e1 = cov_ptr[k + 1];
+    const int64_t c0 = (int64_t)blockIdx.y * cols_per_block;
+    const int64_t c1 = c0 + cols_per_block < ncols ? c0 + cols_per_block : ncols;
+    for (int64_t col = c0; col < c1; ++col) {
+        const double *d = D + col * (int64_t)ldD;
+        double s = 0.0;
+        for (int64_t e = e0; e < e1; ++e) {
+            const CoverEntry en = ent[e];
+            const int P = en.pofs_p & 0xff;
+            const double *dj = d + (en.pofs_p >> 8);
+            const double *ch = chi + en.chi_off;
+            for (int q = 0; q < P; ++q) s = fma(ch[(int64_t)q * en.n_j], dj[q], s);
+        }
+        Out[i + col * ldo] += s;
+    }
+}
+
+}  // namespace
+
+int launch_nl_project(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, int64_t ncols, double scale, double *D,
+                      cudaStream_t st)
+{
+    const int cols_per_cta = NLP_WARPS * NLP_COLS;
+    const int64_t max_y = 65535;
+    for (int64_t j0 = 0; j0 < ncols; j0 += max_y * cols_per_cta) {
+        const int64_t nb = std::min<int64_t>(ncols - j0, max_y * cols_per_cta);
+        dim3 grid((unsigned)ctx->n_atoms, (unsigned)((nb + cols_per_cta - 1) / cols_per_cta));
+        const double *Xb = X + j0 * ldx;
+        double *Db = D + j0 * (int64_t)ctx->n_proj_total;
+#define NLP_LAUNCH(PM)                                                                                         \
+        nl_project_kernel<PM><<<grid, NLP_WARPS * 32, 0, st>>>(ctx->d_supp_ptr, ctx->d_supp_idx, ctx->d_n_proj, \
+            ctx->d_proj_ofs, ctx->d_chi_ptr, ctx->d_chi, ctx->d_gamma, Xb, ldx, nb, scale, Db, ctx->n_proj_total)
+        if (ctx->max_proj <= 4) NLP_LAUNCH(4);
+        else if (ctx->max_proj <= 9) NLP_LAUNCH(9);
+        else NLP_LAUNCH(16);
+#undef NLP_LAUNCH
+        ctx->kernel_launches++;
+    }
+    SPARC_CUDA_TRY(cudaGetLastError());
+    return SPARC_GPU_SUCCESS;
+}
+
+int launch_nl_pull(sparc_gpu_ctx *ctx, const double *D, double *Out, int64_t ldo, int64_t ncols, cudaStream_t st)
+{
+    if (ctx->n_covered == 0) return SPARC_GPU_SUCCESS;
+    const int64_t bx = (ctx->n_covered + 127) / 128;
+    // enough CTAs to fill the chip, but keep the (entry, chi) re-reads per thread amortised over columns
+    int cols_per_block = 16;
+    int64_t by = (ncols + cols_per_block - 1) / cols_per_block;
+    while (by > 65535) { cols_per_block *= 2; by = (ncols + cols_per_block - 1) / cols_per_block; }
+    dim3 grid((unsigned)bx, (unsigned)by);
+    nl_pull_kernel<<<grid, 128, 0, st>>>(ctx->d_cov_idx, ctx->d_cov_ptr, ctx->d_cov_ent, ctx->d_chi, D,
+                                         ctx->n_proj_total, Out, ldo, ctx->n_covered, ncols, cols_per_block);
+    ctx->kernel_launches++;
+    SPARC_CUDA_TRY(cudaGetLastError());
+    return SPARC_GPU_SUCCESS;
+}
