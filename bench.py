@@ -1,0 +1,333 @@
+#!/usr/bin/env python
+"""bench.py -- one CheFSI step (filter -> project -> rotate) on a synthetic workload, on N B200s.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path: Chebyshev filter of degree m on the
+N_d x N_s block, Hs = Psi^T H Psi, Ms = Psi^T Psi, and the in-place rotation Psi <- Psi Q, all through the
+C ABI (include/sparc_gpu.h).  The headline `value` is BASELINE.json's metric: filter throughput in
+grid-pt*orbital*degree/s (N_d*N_s*m / filter time); `hbm_gbs` (x24 B) and `subspace_tflops` are the other two
+parts of that compound metric.  Default workload: BASELINE.json configs[1] (48^3, N_s = 256, degree 20).
+
+N > 1: the path shards by orbital columns with no data-path collective for the filter;
+this build runs N independent replicas of the workload ("replicas only") and reports
+the aggregate, scaling = "weak".
+
+--impl reference times the CPU oracle (oracle/, acc_t = double build) on the host cores: a deliberately slow
+program, reported as context.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "CheFSI filter grid-pt·orbital·degree/s + HBM GB/s; subspace FP64 TFLOP/s"
+UNIT = "grid-pt*orbital*degree/s"
+ALG_BYTES_PER_UNIT = 24.0       # read Psi_k, read Psi_{k-1}, write Psi_{k+1}
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` capture (profiles/r01_ncu_stencil_tma_cfg1.md).  None until captured.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {1: None}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+
+    FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+              "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device_index: int):
+        self.dev = device_index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits", "-lms", "200",
+                 "-i", str(self.dev)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons = [], None, set()
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); smax = float(f[2])
+            except ValueError:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": smax,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_filter_rate(wl, ncols, acc="f64"):
+    """Time the CPU oracle's Chebyshev filter on `ncols` columns; returns (units/s, seconds, threads)."""
+    from oracle import oracle as orc
+    H = orc.Hamiltonian(wl, acc=acc)
+    X = wl.psi_columns(range(ncols))
+    t0 = time.perf_counter()
+    H.chebyshev_filter(X, wl.degree, wl.a, wl.b, wl.a0)
+    dt = time.perf_counter() - t0
+    return wl.nd * ncols * wl.degree / dt, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2302_09708_b200 import workloads as wlmod
+    from oracle import oracle as orc
+    orc.build()
+    cores = os.cpu_count() or 1
+    wl = wlmod.make_workload(args.config)
+    ncols = max(1, min(wl.ns, cores))
+    times = []
+    for i in range(args.warmup + args.steps):
+        rate, dt = oracle_filter_rate(wl, ncols)
+        if i >= args.warmup:
+            times.append(dt)
+    dt = sum(times) / len(times)
+    value = wl.nd * ncols * wl.degree / dt
+    sample = (f"Chebyshev filter (degree {wl.degree}) of {ncols} of the {wl.ns} columns of {wl.name} per step, "
+              f"OpenMP over columns")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl.name, "nd": wl.nd, "ns": wl.ns, "degree": wl.degree, "sample_columns": ncols},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores,
+                         "kind": "oracle (oracle/chefsi_oracle.c, acc_t=double build)", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    from paper_2302_09708_b200 import api, workloads as wlmod
+
+    wl = wlmod.make_workload(args.config)
+    g = api.SparcGpu(wl, device=local_rank)
+    nd, ns, m = wl.nd, wl.ns, wl.degree
+    ld = nd
+    psi0 = torch.empty((ns, ld), dtype=torch.float64, device=dev)
+    api.fill_uniform(psi0, wl.seed, wlmod.STREAM_PSI, 0, -1.0, 1.0)
+    psi = torch.empty_like(psi0)
+    Q = api.colmajor_from_numpy(wl.q_matrix(), device=dev)
+    Hs = torch.empty((ns, ns), dtype=torch.float64, device=dev)
+    Ms = torch.empty_like(Hs)
+    col_block = args.col_block if args.col_block else wl.col_block
+
+    def ev():
+        return torch.cuda.Event(enable_timing=True)
+
+    def one_step(timers=None):
+        psi.copy_(psi0)                       # refill (also sweeps L2: 226 MB > 126 MB); outside the timers
+        e = [ev() for _ in range(4)] if timers is not None else None
+        if e: e[0].record()
+        g.chebyshev_filter(psi, m, wl.a, wl.b, wl.a0, col_block=col_block)
+        if e: e[1].record()
+        g.project(psi, col_block=col_block, Hs=Hs, Ms=Ms)
+        if e: e[2].record()
+        g.rotate(psi, Q)
+        if e: e[3].record()
+        if timers is not None:
+            timers.append(e)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        one_step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    launches0 = g.get_info("kernel_launches")
+    timers = []
+    t_wall0 = time.perf_counter()
+    for _ in range(args.steps):
+        one_step(timers)
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    launches = g.get_info("kernel_launches") - launches0
+    clocks = sampler.stop() if rank == 0 else None
+
+    filt = sum(e[0].elapsed_time(e[1]) for e in timers) / args.steps
+    proj = sum(e[1].elapsed_time(e[2]) for e in timers) / args.steps
+    rot = sum(e[2].elapsed_time(e[3]) for e in timers) / args.steps
+    t = torch.tensor([filt, proj, rot], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    filt, proj, rot = (float(x) for x in t.cpu())
+    step_ms = filt + proj + rot
+
+    # ---- end to end: host buffers, H2D + filter + D2H through the same C-ABI call ---------------------------
+    host_in = torch.empty((ns, ld), dtype=torch.float64).pin_memory()
+    host_in.copy_(psi0)
+    host_out = torch.empty((ns, ld), dtype=torch.float64).pin_memory()
+    e2e_times = []
+    for i in range(1 + min(args.steps, 3)):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        psi.copy_(host_in, non_blocking=True)
+        g.chebyshev_filter(psi, m, wl.a, wl.b, wl.a0, col_block=col_block)
+        host_out.copy_(psi, non_blocking=True)
+        torch.cuda.synchronize()
+        if i > 0:
+            e2e_times.append(time.perf_counter() - t0)
+    te = torch.tensor([sum(e2e_times) / len(e2e_times)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_s = float(te.cpu()[0])
+    del host_in, host_out
+
+    # ---- roofline of the dominant kernel: per-launch CUDA events inside the library, same launch config ------
+    roofline = None
+    kinds = {0: "stencil_generic", 1: "stencil_tma", 2: "nl_project", 3: "nl_pull", 4: "gemm_tn", 5: "gemm_nn",
+             6: "splitk_reduce", 7: "copy2d"}
+    share = {}
+    if rank == 0:
+        g.set_option("profile_reset", 1)
+        g.set_option("profile", 1)
+        for _ in range(2):
+            psi.copy_(psi0)
+            g.chebyshev_filter(psi, m, wl.a, wl.b, wl.a0, col_block=col_block)
+        torch.cuda.synchronize()
+        g.set_option("profile", 0)
+        prof = {k: (g.get_info(f"prof_ns:{k}"), g.get_info(f"prof_count:{k}")) for k in kinds}
+        tot = sum(v[0] for v in prof.values()) or 1
+        share = {kinds[k]: round(v[0] / tot, 4) for k, v in prof.items() if v[1]}
+        sk = 1 if prof[1][1] else 0
+        ns_total, n_launch = prof[sk]
+        cb = col_block if col_block and col_block > 0 else min(ns, 1024)
+        nblocks = (ns + cb - 1) // cb
+        # per filter call: each column block launches 1 kernel without Prev (16 B/pt) and m-1 with Prev (24 B/pt)
+        alg_bytes = 2 * nd * ns * (16.0 + 24.0 * (m - 1))
+        achieved = alg_bytes / (ns_total * 1e-9) / 1e9 if ns_total else 0.0
+        peak, peak_src = measured_peaks()
+        traffic = NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.config)
+        roofline = {"bound": "hbm", "kernel": kinds[sk], "achieved": achieved, "peak": peak, "unit": "GB/s",
+                    "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                    "launches_timed": n_launch, "avg_launch_us": ns_total / max(n_launch, 1) / 1e3,
+                    "alg_bytes_per_launch": alg_bytes / max(n_launch, 1),
+                    "filter_time_share_by_kernel": share}
+
+    # ---- CPU oracle beside it (rank 0, N = 1 only) --------------------------------------------------------
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        from oracle import oracle as orc
+        orc.build()
+        cores = os.cpu_count() or 1
+        ncols = max(1, min(ns, cores))
+        rate, dt = oracle_filter_rate(wl, ncols)
+        while dt < 8.0 and ncols * 2 <= ns:
+            ncols *= 2
+            rate, dt = oracle_filter_rate(wl, ncols)
+        cpu_baseline = {"value": rate, "unit": UNIT, "cores": cores,
+                        "kind": "oracle (oracle/chefsi_oracle.c, acc_t=double build)",
+                        "sample": f"Chebyshev filter degree {m} on {ncols} of {ns} columns of {wl.name}: {dt:.1f} s",
+                        }
+
+    if rank == 0:
+        units = float(nd) * ns * m * world
+        value = units / (filt * 1e-3)
+        sub_flops = 3 * 2.0 * nd * ns * ns * world
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "grid": list(wl.n), "nd": nd, "ns": ns, "degree": m,
+                       "atoms": wl.n_atoms, "col_block": col_block, "parallelism": f"replicas x{world}",
+                       "l2": "Psi block (226 MB at cfg1) is larger than L2 and is refilled between steps"},
+            "hbm_gbs": value * ALG_BYTES_PER_UNIT / 1e9,
+            "subspace_tflops": sub_flops / ((proj + rot) * 1e-3) / 1e12,
+            "step_ms": {"filter": filt, "project": proj, "rotate": rot, "wall_per_step": t_wall / args.steps * 1e3},
+            "clocks": clocks,
+            "e2e": {"value": units / e2e_s, "unit": UNIT, "h2d_bytes_per_step": ns * ld * 8,
+                    "d2h_bytes_per_step": ns * ld * 8,
+                    "what": "pinned host Psi -> H2D -> sparc_gpu_chebyshev_filter -> D2H, wall clock"},
+            "gpu_launches": int(launches),
+            "roofline": roofline,
+            "cpu_baseline": cpu_baseline,
+        }
+        print(json.dumps(line))
+    g.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--col-block", type=int, default=0)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -12,7 +12,58 @@
 
 #include "internal.h"
 
+struct ProfRec { int kind; cudaEvent_t a, b; };
+struct ProfState {
+    bool on = false;
+    std::vector<ProfRec> recs;
+    std::vector<cudaEvent_t> pool;
+    double ns[KK_COUNT] = {0};
+    int64_t count[KK_COUNT] = {0};
+    cudaEvent_t cur = nullptr;
+};
+
+void prof_begin(sparc_gpu_ctx *ctx, int kind, cudaStream_t st)
+{
+    ctx->kernel_launches++;
+    ProfState *p = ctx->prof;
+    if (!p) return;
+    p->count[kind]++;
+    if (!p->on) return;
+    cudaEvent_t a;
+    if (p->pool.empty()) { if (cudaEventCreate(&a) != cudaSuccess) { (void)cudaGetLastError(); p->cur = nullptr; return; } }
+    else { a = p->pool.back(); p->pool.pop_back(); }
+    cudaEventRecord(a, st);
+    p->cur = a;
+}
+
+void prof_end(sparc_gpu_ctx *ctx, int kind, cudaStream_t st)
+{
+    ProfState *p = ctx->prof;
+    if (!p || !p->on || !p->cur) return;
+    cudaEvent_t b;
+    if (p->pool.empty()) { if (cudaEventCreate(&b) != cudaSuccess) { (void)cudaGetLastError(); return; } }
+    else { b = p->pool.back(); p->pool.pop_back(); }
+    cudaEventRecord(b, st);
+    p->recs.push_back({kind, p->cur, b});
+    p->cur = nullptr;
+}
+
 namespace {
+
+// fold finished event pairs into the per-kind totals (caller has synchronised the stream)
+void prof_collect(ProfState *p)
+{
+    for (auto &r : p->recs) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(r.b) == cudaSuccess && cudaEventElapsedTime(&ms, r.a, r.b) == cudaSuccess)
+            p->ns[r.kind] += (double)ms * 1e6;
+        else
+            (void)cudaGetLastError();
+        p->pool.push_back(r.a);
+        p->pool.push_back(r.b);
+    }
+    p->recs.clear();
+}
 
 // O(1) host arithmetic: central FD weights of the second derivative, radius r (R1).
 void fd_weights_host(int r, double *w)
@@ -194,6 +245,7 @@ int sparc_gpu_create(const sparc_gpu_desc *desc, sparc_gpu_ctx **out)
     c->radius = desc->fd_order / 2;
     c->nd = (int64_t)desc->n[0] * desc->n[1] * desc->n[2];
     c->opt_nonlocal = 1;
+    c->prof = new (std::nothrow) ProfState();
     fd_weights_host(c->radius, c->w);
     double isum = 0.0;
     for (int p = 0; p <= SPARC_MAX_RADIUS; ++p) { c->coef.cx[p] = c->coef.cy[p] = c->coef.cz[p] = 0.0; }
@@ -273,7 +325,7 @@ int sparc_gpu_create(const sparc_gpu_desc *desc, sparc_gpu_ctx **out)
         if ((st = upload(&c->d_cov_ptr, cov_ptr.data(), cov_ptr.size()))) break;
         if ((st = upload(&c->d_cov_ent, ent.data(), ent.size()))) break;
     } while (0);
-    if (st != SPARC_GPU_SUCCESS) { (void)cudaGetLastError(); free_tables(c); delete c; return st; }
+    if (st != SPARC_GPU_SUCCESS) { (void)cudaGetLastError(); free_tables(c); delete c->prof; delete c; return st; }
     *out = c;
     return SPARC_GPU_SUCCESS;
 }
@@ -283,6 +335,11 @@ int sparc_gpu_destroy(sparc_gpu_ctx *ctx)
     if (!ctx) return SPARC_GPU_INVALID_ARG;
     cudaSetDevice(ctx->device);
     free_tables(ctx);
+    if (ctx->prof) {
+        prof_collect(ctx->prof);
+        for (auto e : ctx->prof->pool) cudaEventDestroy(e);
+        delete ctx->prof;
+    }
     delete ctx;
     return SPARC_GPU_SUCCESS;
 }
@@ -300,6 +357,13 @@ int sparc_gpu_set_option(sparc_gpu_ctx *ctx, const char *key, int64_t value)
     if (!ctx || !key) return SPARC_GPU_INVALID_ARG;
     if (!strcmp(key, "stencil_path")) { if (value < 0 || value > 2) return SPARC_GPU_INVALID_ARG; ctx->opt_stencil_path = (int)value; return 0; }
     if (!strcmp(key, "nonlocal")) { ctx->opt_nonlocal = value ? 1 : 0; return 0; }
+    if (!strcmp(key, "profile")) { if (!ctx->prof) return SPARC_GPU_OUT_OF_MEMORY; ctx->prof->on = value != 0; return 0; }
+    if (!strcmp(key, "profile_reset")) {
+        if (!ctx->prof) return SPARC_GPU_OUT_OF_MEMORY;
+        prof_collect(ctx->prof);
+        for (int k = 0; k < KK_COUNT; ++k) { ctx->prof->ns[k] = 0; ctx->prof->count[k] = 0; }
+        return 0;
+    }
     if (!strcmp(key, "gemm_path")) { if (value < 0 || value > 2) return SPARC_GPU_INVALID_ARG; ctx->opt_gemm_path = (int)value; return 0; }
     return SPARC_GPU_INVALID_ARG;
 }
@@ -313,6 +377,15 @@ int sparc_gpu_get_info(const sparc_gpu_ctx *ctx, const char *key, int64_t *value
     if (!strcmp(key, "covered_points")) { *value = ctx->n_covered; return 0; }
     if (!strcmp(key, "stencil_path_last")) { *value = ctx->stencil_path_last; return 0; }
     if (!strcmp(key, "sm_count")) { *value = ctx->sm_count; return 0; }
+    if (!strncmp(key, "prof_ns:", 8) || !strncmp(key, "prof_count:", 11)) {
+        if (!ctx->prof) return SPARC_GPU_OUT_OF_MEMORY;
+        const bool is_ns = key[5] == 'n';
+        const int kind = atoi(key + (is_ns ? 8 : 11));
+        if (kind < 0 || kind >= KK_COUNT) return SPARC_GPU_INVALID_ARG;
+        if (is_ns) { prof_collect(ctx->prof); *value = (int64_t)ctx->prof->ns[kind]; }
+        else *value = ctx->prof->count[kind];
+        return 0;
+    }
     return SPARC_GPU_INVALID_ARG;
 }
 

@@ -207,16 +207,19 @@ int launch_dmma(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const double *
     dim3 grid((unsigned)(tiles_m * tiles_n), 1, (unsigned)plan.splits);
     const bool vec = aligned16(A) && aligned16(B) && (lda % 2 == 0) && (ldb % 2 == 0);
     const size_t smem = smem_bytes(A_MMAJOR);
+    const int kind = A_MMAJOR ? KK_GEMM_NN : KK_GEMM_TN;
     if (vec) {
         auto kern = gemm_dmma_kernel<A_MMAJOR, true>;
         SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        prof_begin(ctx, kind, st);
         kern<<<grid, GEMM_THREADS, smem, st>>>(A, lda, B, ldb, C, ldc, M, N, K, plan.k_chunk, tiles_m);
     } else {
         auto kern = gemm_dmma_kernel<A_MMAJOR, false>;
         SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        prof_begin(ctx, kind, st);
         kern<<<grid, GEMM_THREADS, smem, st>>>(A, lda, B, ldb, C, ldc, M, N, K, plan.k_chunk, tiles_m);
     }
-    ctx->kernel_launches++;
+    prof_end(ctx, kind, st);
     SPARC_CUDA_TRY(cudaGetLastError());
     return SPARC_GPU_SUCCESS;
 }
@@ -235,8 +238,9 @@ int launch_gemm_tn(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const doubl
     if (M <= 0 || N <= 0) return SPARC_GPU_SUCCESS;
     if (ctx->opt_gemm_path == 1) {
         const int64_t blocks = (M * N + 255) / 256;
+        prof_begin(ctx, KK_GEMM_TN, st);
         gemm_simple_kernel<false><<<(unsigned)blocks, 256, 0, st>>>(A, lda, B, ldb, C, ldc, M, N, K);
-        ctx->kernel_launches++;
+        prof_end(ctx, KK_GEMM_TN, st);
         SPARC_CUDA_TRY(cudaGetLastError());
         return SPARC_GPU_SUCCESS;
     }
@@ -245,8 +249,9 @@ int launch_gemm_tn(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const doubl
         double *part = (double *)ws;
         SPARC_TRY(launch_dmma<false>(ctx, A, lda, B, ldb, part, M, M, N, K, plan, st));
         int64_t blocks = std::min<int64_t>((M * N + 255) / 256, (int64_t)ctx->sm_count * 8);
+        prof_begin(ctx, KK_SPLITK_REDUCE, st);
         splitk_reduce_kernel<<<(unsigned)blocks, 256, 0, st>>>(part, plan.splits, M, N, C, ldc);
-        ctx->kernel_launches++;
+        prof_end(ctx, KK_SPLITK_REDUCE, st);
         SPARC_CUDA_TRY(cudaGetLastError());
         return SPARC_GPU_SUCCESS;
     }
@@ -259,8 +264,9 @@ int launch_gemm_nn(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const doubl
     if (M <= 0 || N <= 0) return SPARC_GPU_SUCCESS;
     if (ctx->opt_gemm_path == 1) {
         const int64_t blocks = (M * N + 255) / 256;
+        prof_begin(ctx, KK_GEMM_NN, st);
         gemm_simple_kernel<true><<<(unsigned)blocks, 256, 0, st>>>(A, lda, B, ldb, C, ldc, M, N, K);
-        ctx->kernel_launches++;
+        prof_end(ctx, KK_GEMM_NN, st);
         SPARC_CUDA_TRY(cudaGetLastError());
         return SPARC_GPU_SUCCESS;
     }

@@ -63,7 +63,18 @@ struct sparc_gpu_ctx {
     int stencil_path_last;
     // driver entry point for tensor-map encoding (resolved at create; NULL if unavailable)
     void *fn_encode_tiled;
+    // optional per-kernel CUDA-event timing (option "profile"); NULL when off
+    struct ProfState *prof;
 };
+
+// Kernel kinds for the event profiler and the launch counters.
+enum KernelKind {
+    KK_STENCIL_GENERIC = 0, KK_STENCIL_TMA = 1, KK_NL_PROJECT = 2, KK_NL_PULL = 3, KK_GEMM_TN = 4,
+    KK_GEMM_NN = 5, KK_SPLITK_REDUCE = 6, KK_COPY2D = 7, KK_COUNT = 8
+};
+// Bracket one kernel launch with events when profiling is on (no-ops otherwise); both bump the counters.
+void prof_begin(sparc_gpu_ctx *ctx, int kind, cudaStream_t st);
+void prof_end(sparc_gpu_ctx *ctx, int kind, cudaStream_t st);
 
 #define SPARC_CUDA_TRY(expr)                                         \
     do {                                                             \

@@ -115,11 +115,12 @@ int launch_nl_project(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, int64_t 
 #define NLP_LAUNCH(PM)                                                                                         \
         nl_project_kernel<PM><<<grid, NLP_WARPS * 32, 0, st>>>(ctx->d_supp_ptr, ctx->d_supp_idx, ctx->d_n_proj, \
             ctx->d_proj_ofs, ctx->d_chi_ptr, ctx->d_chi, ctx->d_gamma, Xb, ldx, nb, scale, Db, ctx->n_proj_total)
+        prof_begin(ctx, KK_NL_PROJECT, st);
         if (ctx->max_proj <= 4) NLP_LAUNCH(4);
         else if (ctx->max_proj <= 9) NLP_LAUNCH(9);
         else NLP_LAUNCH(16);
 #undef NLP_LAUNCH
-        ctx->kernel_launches++;
+        prof_end(ctx, KK_NL_PROJECT, st);
     }
     SPARC_CUDA_TRY(cudaGetLastError());
     return SPARC_GPU_SUCCESS;
@@ -134,9 +135,10 @@ int launch_nl_pull(sparc_gpu_ctx *ctx, const double *D, double *Out, int64_t ldo
     int64_t by = (ncols + cols_per_block - 1) / cols_per_block;
     while (by > 65535) { cols_per_block *= 2; by = (ncols + cols_per_block - 1) / cols_per_block; }
     dim3 grid((unsigned)bx, (unsigned)by);
+    prof_begin(ctx, KK_NL_PULL, st);
     nl_pull_kernel<<<grid, 128, 0, st>>>(ctx->d_cov_idx, ctx->d_cov_ptr, ctx->d_cov_ent, ctx->d_chi, D,
                                          ctx->n_proj_total, Out, ldo, ctx->n_covered, ncols, cols_per_block);
-    ctx->kernel_launches++;
+    prof_end(ctx, KK_NL_PULL, st);
     SPARC_CUDA_TRY(cudaGetLastError());
     return SPARC_GPU_SUCCESS;
 }

@@ -96,9 +96,10 @@ int launch_stencil_generic(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, dou
         int64_t bx = (ctx->nd + 255) / 256;
         if (bx > 4096) bx = 4096;
         dim3 grid((unsigned)bx, (unsigned)nb);
+        prof_begin(ctx, KK_STENCIL_GENERIC, st);
         stencil_generic_kernel<<<grid, 256, 0, st>>>(P, ctx->d_veff, X + j0 * ldx, ldx, Out + j0 * ldo, ldo,
                                                      (beta != 0.0 && Prev) ? Prev + j0 * ldp : nullptr, ldp);
-        ctx->kernel_launches++;
+        prof_end(ctx, KK_STENCIL_GENERIC, st);
     }
     SPARC_CUDA_TRY(cudaGetLastError());
     return SPARC_GPU_SUCCESS;
@@ -110,8 +111,9 @@ int launch_copy_2d(sparc_gpu_ctx *ctx, double *dst, int64_t ldd, const double *s
     if (rows <= 0 || cols <= 0) return SPARC_GPU_SUCCESS;
     int64_t blocks = (rows * cols + 255) / 256;
     if (blocks > (int64_t)ctx->sm_count * 32) blocks = (int64_t)ctx->sm_count * 32;
+    prof_begin(ctx, KK_COPY2D, st);
     copy_2d_kernel<<<(unsigned)blocks, 256, 0, st>>>(dst, ldd, src, lds, rows, cols);
-    ctx->kernel_launches++;
+    prof_end(ctx, KK_COPY2D, st);
     SPARC_CUDA_TRY(cudaGetLastError());
     return SPARC_GPU_SUCCESS;
 }
