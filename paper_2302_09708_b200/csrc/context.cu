@@ -196,8 +196,12 @@ int h_pass(sparc_gpu_ctx *c, const double *X, int64_t ldx, double *Out, int64_t 
     }
     c->stencil_path_last = path;
     if (c->opt_nonlocal && c->n_atoms > 0 && c->n_proj_total > 0 && c->supp_total > 0) {
-        SPARC_TRY(launch_nl_project(c, X, ldx, ncols, alpha, D, st));
-        SPARC_TRY(launch_nl_pull(c, D, Out, ldo, ncols, st));
+        if (c->opt_nonlocal_mode == 1) {
+            SPARC_TRY(launch_nl_project(c, X, ldx, ncols, alpha, D, st));
+            SPARC_TRY(launch_nl_pull(c, D, Out, ldo, ncols, st));
+        } else {
+            SPARC_TRY(launch_nl_fused(c, X, ldx, Out, ldo, ncols, alpha, st));
+        }
     }
     return SPARC_GPU_SUCCESS;
 }
@@ -356,6 +360,7 @@ int sparc_gpu_set_option(sparc_gpu_ctx *ctx, const char *key, int64_t value)
 {
     if (!ctx || !key) return SPARC_GPU_INVALID_ARG;
     if (!strcmp(key, "stencil_path")) { if (value < 0 || value > 2) return SPARC_GPU_INVALID_ARG; ctx->opt_stencil_path = (int)value; return 0; }
+    if (!strcmp(key, "nonlocal_mode")) { if (value < 0 || value > 1) return SPARC_GPU_INVALID_ARG; ctx->opt_nonlocal_mode = (int)value; return 0; }
     if (!strcmp(key, "nonlocal")) { ctx->opt_nonlocal = value ? 1 : 0; return 0; }
     if (!strcmp(key, "profile")) { if (!ctx->prof) return SPARC_GPU_OUT_OF_MEMORY; ctx->prof->on = value != 0; return 0; }
     if (!strcmp(key, "profile_reset")) {
@@ -364,6 +369,10 @@ int sparc_gpu_set_option(sparc_gpu_ctx *ctx, const char *key, int64_t value)
         for (int k = 0; k < KK_COUNT; ++k) { ctx->prof->ns[k] = 0; ctx->prof->count[k] = 0; }
         return 0;
     }
+    if (!strcmp(key, "stencil_ay")) { ctx->opt_stencil_ay = (int)value; return 0; }
+    if (!strcmp(key, "stencil_ty")) { ctx->opt_stencil_ty = (int)value; return 0; }
+    if (!strcmp(key, "stencil_stages")) { ctx->opt_stencil_stages = (int)value; return 0; }
+    if (!strcmp(key, "stencil_zchunks")) { ctx->opt_stencil_zchunks = (int)value; return 0; }
     if (!strcmp(key, "gemm_path")) { if (value < 0 || value > 2) return SPARC_GPU_INVALID_ARG; ctx->opt_gemm_path = (int)value; return 0; }
     return SPARC_GPU_INVALID_ARG;
 }

@@ -58,6 +58,11 @@ struct sparc_gpu_ctx {
     int opt_stencil_path;      // 0 auto, 1 generic, 2 TMA
     int opt_nonlocal;          // 1 on
     int opt_gemm_path;         // 0 auto, 1 simple, 2 DMMA
+    int opt_nonlocal_mode;     // 0 fused per-atom kernel with atomic scatter, 1 project + pull (deterministic)
+    int opt_stencil_ay;        // 0 auto, 1 or 2: rows per consumer thread of the TMA stencil kernel
+    int opt_stencil_ty;        // 0 auto, else forced tile rows of the TMA stencil kernel
+    int opt_stencil_stages;    // 0 auto, else cap on the smem ring depth
+    int opt_stencil_zchunks;   // 0 auto, else forced number of z chunks
     // counters
     mutable int64_t kernel_launches;
     int stencil_path_last;
@@ -70,7 +75,7 @@ struct sparc_gpu_ctx {
 // Kernel kinds for the event profiler and the launch counters.
 enum KernelKind {
     KK_STENCIL_GENERIC = 0, KK_STENCIL_TMA = 1, KK_NL_PROJECT = 2, KK_NL_PULL = 3, KK_GEMM_TN = 4,
-    KK_GEMM_NN = 5, KK_SPLITK_REDUCE = 6, KK_COPY2D = 7, KK_COUNT = 8
+    KK_GEMM_NN = 5, KK_SPLITK_REDUCE = 6, KK_COPY2D = 7, KK_NL_FUSED = 8, KK_COUNT = 9
 };
 // Bracket one kernel launch with events when profiling is on (no-ops otherwise); both bump the counters.
 void prof_begin(sparc_gpu_ctx *ctx, int kind, cudaStream_t st);
@@ -112,6 +117,11 @@ int launch_nl_project(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, int64_t 
 // Out[i, col] += sum_{(J,t) covering i} sum_q chi_J[t, q] D[ofs_J + q, col]
 int launch_nl_pull(sparc_gpu_ctx *ctx, const double *D, double *Out, int64_t ldo, int64_t ncols,
                    cudaStream_t st);
+
+// Out[idx_J, col] += scale * chi_J diag(gamma_J) chi_J^T X[idx_J, col] for every atom J: fused gather / GEMM / atomic
+// scatter (default nonlocal path; not bitwise reproducible across runs, see option "nonlocal_mode")
+int launch_nl_fused(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double *Out, int64_t ldo, int64_t ncols,
+                    double scale, cudaStream_t st);
 
 // C (M x N, col-major, ldc) = A^T B, A: K x M (lda), B: K x N (ldb), contraction over K rows.
 // ws: split-K partials (gemm_tn_ws_bytes).  symmetric_out: A == B, fill lower from upper.

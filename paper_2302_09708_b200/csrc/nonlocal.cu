@@ -100,6 +100,155 @@ nl_pull_kernel(const int32_t *__restrict__ cov_idx, const int64_t *__restrict__ 
     }
 }
 
+
+// ---- fused per-atom kernel (default path) ---------------------------------------------------------------------
+// One CTA = one atom J x NLF_WARPS*NCW columns.  The chi_J rows and support indices are streamed through a
+// double-buffered shared-memory tile (cp.async) that all warps of the CTA share; each warp owns NCW columns.
+//   pass 1 (gather + small GEMM): lanes stride over the support rows t, gather X[idx[t], col] (coalesced along the
+//           x-runs of the support) and accumulate C[q][c] += chi[t][q] X[idx[t]][c] in registers; a butterfly
+//           all-reduce leaves D[q][c] = scale * gamma[q] * C[q][c] in every lane.
+//   pass 2 (small GEMM + scatter): the tile stream is replayed (chi_J comes from L2) and each lane adds
+//           sum_q chi[t][q] D[q][c] to Out[idx[t]][c] with an FP64 atomic add (RED): supports of different atoms
+//           overlap, the atomics make the scatter conflict-free (north_star: "coloured or atomic").
+constexpr int NLF_WARPS = 8;
+
+__device__ __forceinline__ void cp_async8(void *smem, const void *gmem, int src_bytes)
+{
+    unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(sa), "l"(gmem), "r"(src_bytes));
+}
+__device__ __forceinline__ void cp_async4(void *smem, const void *gmem, int src_bytes)
+{
+    unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;\n" ::"r"(sa), "l"(gmem), "r"(src_bytes));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::); }
+
+template <int PMAX, int NCW, int NLF_TILE>      // NLF_TILE: support rows per shared-memory tile
+__global__ void __launch_bounds__(NLF_WARPS * 32)
+nl_fused_kernel(const int64_t *__restrict__ supp_ptr, const int32_t *__restrict__ supp_idx,
+                const int32_t *__restrict__ n_proj, const int32_t *__restrict__ proj_ofs,
+                const int64_t *__restrict__ chi_ptr, const double *__restrict__ chi,
+                const double *__restrict__ gamma, const double *__restrict__ X, int64_t ldx, double *Out, int64_t ldo,
+                int64_t ncols, double scale)
+{
+    __shared__ __align__(16) double chi_s[2][PMAX][NLF_TILE];
+    __shared__ int32_t idx_s[2][NLF_TILE];
+    const int J = blockIdx.x;
+    const int P = n_proj[J];
+    const int64_t s0 = supp_ptr[J];
+    const int nJ = (int)(supp_ptr[J + 1] - s0);
+    if (P == 0 || nJ == 0) return;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int64_t col0 = ((int64_t)blockIdx.y * NLF_WARPS + warp) * NCW;
+    const bool warp_active = col0 < ncols;          // inactive warps still help loading tiles
+    const int32_t *idx = supp_idx + s0;
+    const double *ch = chi + chi_ptr[J];
+    const int ntiles = (nJ + NLF_TILE - 1) / NLF_TILE;
+
+    auto load_tile = [&](int tile, int buf) {
+        const int t0 = tile * NLF_TILE;
+        for (int k = tid; k < NLF_TILE; k += NLF_WARPS * 32) {
+            const int t = t0 + k;
+            const bool ok = t < nJ;
+            cp_async4(&idx_s[buf][k], ok ? idx + t : idx, ok ? 4 : 0);
+#pragma unroll
+            for (int q = 0; q < PMAX; ++q)
+                if (q < P) cp_async8(&chi_s[buf][q][k], ok ? ch + t + (int64_t)q * nJ : ch, ok ? 8 : 0);
+        }
+        cp_async_commit();
+    };
+
+    const double *xc[NCW];
+    double *oc[NCW];
+#pragma unroll
+    for (int c = 0; c < NCW; ++c) {
+        const int64_t col = (col0 + c < ncols) ? col0 + c : (warp_active ? col0 : 0);
+        xc[c] = X + col * ldx;
+        oc[c] = Out + col * ldo;
+    }
+
+    double acc[PMAX][NCW];
+#pragma unroll
+    for (int q = 0; q < PMAX; ++q)
+#pragma unroll
+        for (int c = 0; c < NCW; ++c) acc[q][c] = 0.0;
+
+    // ---- pass 1: C = chi^T X[idx] -----------------------------------------------------------------------------
+    load_tile(0, 0);
+    for (int tile = 0; tile < ntiles; ++tile) {
+        const int buf = tile & 1;
+        cp_async_wait_all();
+        __syncthreads();
+        if (tile + 1 < ntiles) load_tile(tile + 1, buf ^ 1);
+        if (warp_active) {
+#pragma unroll 2
+            for (int k = lane; k < NLF_TILE; k += 32) {
+                const int i = idx_s[buf][k];          // rows beyond n_J: index 0 with chi = 0
+                double g[NCW];
+#pragma unroll
+                for (int c = 0; c < NCW; ++c) g[c] = __ldg(xc[c] + i);
+#pragma unroll
+                for (int q = 0; q < PMAX; ++q) {
+                    if (q < P) {
+                        const double cv = chi_s[buf][q][k];
+#pragma unroll
+                        for (int c = 0; c < NCW; ++c) acc[q][c] = fma(cv, g[c], acc[q][c]);
+                    }
+                }
+            }
+        }
+    }
+    // butterfly all-reduce: every lane ends with D[q][c] = scale * gamma[q] * sum_t
+    const int po = proj_ofs[J];
+#pragma unroll
+    for (int q = 0; q < PMAX; ++q) {
+        if (q < P) {
+            const double gq = scale * gamma[po + q];
+#pragma unroll
+            for (int c = 0; c < NCW; ++c) {
+                double v = acc[q][c];
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                acc[q][c] = gq * v;
+            }
+        }
+    }
+    // ---- pass 2: Out[idx] += chi D ------------------------------------------------------------------------------
+    __syncthreads();
+    load_tile(0, 0);
+    for (int tile = 0; tile < ntiles; ++tile) {
+        const int buf = tile & 1;
+        cp_async_wait_all();
+        __syncthreads();
+        if (tile + 1 < ntiles) load_tile(tile + 1, buf ^ 1);
+        if (warp_active) {
+            const int t0 = tile * NLF_TILE;
+#pragma unroll 2
+            for (int k = lane; k < NLF_TILE; k += 32) {
+                if (t0 + k < nJ) {
+                    const int i = idx_s[buf][k];
+                    double v[NCW];
+#pragma unroll
+                    for (int c = 0; c < NCW; ++c) v[c] = 0.0;
+#pragma unroll
+                    for (int q = 0; q < PMAX; ++q) {
+                        if (q < P) {
+                            const double cv = chi_s[buf][q][k];
+#pragma unroll
+                            for (int c = 0; c < NCW; ++c) v[c] = fma(cv, acc[q][c], v[c]);
+                        }
+                    }
+#pragma unroll
+                    for (int c = 0; c < NCW; ++c)
+                        if (col0 + c < ncols) atomicAdd(oc[c] + i, v[c]);
+                }
+            }
+        }
+    }
+}
+
 }  // namespace
 
 int launch_nl_project(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, int64_t ncols, double scale, double *D,
@@ -139,6 +288,29 @@ int launch_nl_pull(sparc_gpu_ctx *ctx, const double *D, double *Out, int64_t ldo
     nl_pull_kernel<<<grid, 128, 0, st>>>(ctx->d_cov_idx, ctx->d_cov_ptr, ctx->d_cov_ent, ctx->d_chi, D,
                                          ctx->n_proj_total, Out, ldo, ctx->n_covered, ncols, cols_per_block);
     prof_end(ctx, KK_NL_PULL, st);
+    SPARC_CUDA_TRY(cudaGetLastError());
+    return SPARC_GPU_SUCCESS;
+}
+
+int launch_nl_fused(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double *Out, int64_t ldo, int64_t ncols,
+                    double scale, cudaStream_t st)
+{
+    const int ncw = ctx->max_proj <= 9 ? 4 : 2;
+    const int cols_per_cta = NLF_WARPS * ncw;
+    const int64_t max_y = 65535;
+    for (int64_t j0 = 0; j0 < ncols; j0 += max_y * cols_per_cta) {
+        const int64_t nb = std::min<int64_t>(ncols - j0, max_y * cols_per_cta);
+        dim3 grid((unsigned)ctx->n_atoms, (unsigned)((nb + cols_per_cta - 1) / cols_per_cta));
+#define NLF_LAUNCH(PM, NC, TL)                                                                                       \
+        nl_fused_kernel<PM, NC, TL><<<grid, NLF_WARPS * 32, 0, st>>>(ctx->d_supp_ptr, ctx->d_supp_idx, ctx->d_n_proj,  \
+            ctx->d_proj_ofs, ctx->d_chi_ptr, ctx->d_chi, ctx->d_gamma, X + j0 * ldx, ldx, Out + j0 * ldo, ldo, nb, scale)
+        prof_begin(ctx, KK_NL_FUSED, st);
+        if (ctx->max_proj <= 4) NLF_LAUNCH(4, 4, 256);
+        else if (ctx->max_proj <= 9) NLF_LAUNCH(9, 4, 256);
+        else NLF_LAUNCH(16, 2, 128);
+#undef NLF_LAUNCH
+        prof_end(ctx, KK_NL_FUSED, st);
+    }
     SPARC_CUDA_TRY(cudaGetLastError());
     return SPARC_GPU_SUCCESS;
 }

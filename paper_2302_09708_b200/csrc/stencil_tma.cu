@@ -5,17 +5,18 @@
 //
 // Design (differs from the paper's Micikevicius-style kernel):
 //   * work item = (orbital column, y-tile of TY rows, z-chunk); the tile spans the WHOLE x extent, so the x halo
-//     never leaves the SM; the CTA marches through z.
-//   * warp 0 is the producer: it streams one z-plane of the tile per step into a shared-memory ring with TMA
-//     (cp.async.bulk.tensor.4d over the (x, y, z, column) tensor, boxes of W x 6 rows; out-of-range rows / planes
-//     are zero-filled by TMA = Dirichlet; periodic y / z by wrapping the box coordinate; periodic x by patching the
-//     6+6 halo columns inside shared memory), then hands the plane to the consumers through an mbarrier.
+//     never leaves the SM; the CTA marches through z.  Tiles are small (about 150 consumer threads) so that two or
+//     three CTAs share an SM and overlap each other's pipeline bubbles.
+//   * warp 0 is the producer: one lane streams, per z step, the input plane of the tile (rows y0-6 .. y0+TY+5), the
+//     matching Veff plane and the Prev plane of the output that completes at this step into a shared-memory ring
+//     with TMA (cp.async.bulk.tensor over the (x, y, z, column) tensors); out-of-range rows / planes are
+//     zero-filled by TMA = Dirichlet; periodic y / z by wrapping the box coordinate.  Periodic x needs no halo
+//     columns at all: consumers address their x neighbours through per-thread precomputed (wrapped) offsets.
 //   * the other warps are consumers.  Each thread owns 2 (x) x AY (y) points of the tile and keeps the 13 partial
 //     z-sums of each of them in registers ("register-blocked z-column", accumulate form): an arriving plane adds
 //     its centre/x/y taps to the output plane it is the centre of and one z tap to each of the 12 neighbouring
-//     output planes; the output plane that just received its last tap gets + beta*Prev and is stored.  Shared
-//     memory traffic is 1 + 6/1 + 12/AY vector loads per 2 outputs; coefficients sit in the constant bank.
-//   * Veff and Prev are read straight from global (L2 / HBM) with 16-byte loads, Out is written with 16-byte stores.
+//     output planes; the output plane that just received its last tap gets + beta*Prev and is stored with a
+//     16-byte coalesced store.  Shared-memory traffic is 13 doubles per output; coefficients sit in the constant bank.
 #include <cuda.h>
 
 #include <algorithm>
@@ -26,25 +27,27 @@ namespace {
 
 constexpr int R = 6;             // stencil radius of the tuned path (FD order 12)
 constexpr int NSLOT = 2 * R + 1; // 13 partial sums per point
-constexpr int NSTAGE = 6;        // shared-memory ring depth (planes)
-constexpr int LAG = 2;           // producer refills a stage LAG planes after it was handed out
-constexpr int BOX_ROWS = 6;      // TMA box height (= halo height)
+constexpr int BOX_ROWS = 6;      // TMA box height of the input plane (= halo height)
+constexpr int MAX_THREADS_AY2 = 384;   // 168 registers / thread
+constexpr int MAX_THREADS_AY1 = 320;   // two CTAs of this size per SM -> 102 registers / thread
+constexpr int MAX_STAGES = 8;
 
 struct TmaParams {
     double cx[R + 1], cy[R + 1], cz[R + 1];   // alpha * (-1/2 w_p / h^2)
     double c0a;                                // alpha * (c0 + shift)
     double alpha, beta;
-    const double *veff;
     double *out;
-    const double *prev;
-    int64_t ldo, ldp;
+    int64_t ldo;
     int nx, ny, nz;
-    int W;            // smem row pitch in doubles (>= nx + 12, multiple of 8)
+    int W;            // smem row pitch of the input plane in doubles (multiple of 8)
+    int x_start;      // first x coordinate of the input box: 0 (periodic x) or -6 (Dirichlet x)
     int TY;           // tile rows
     int ntx;          // nx / 2 consumer threads along x
     int n_consumers;  // ntx * (TY / AY)
+    int nstage;
     int ytiles, zchunks, zchunk_len;
     int per_x, per_y, per_z;
+    uint32_t psi_bytes, tile_bytes, stage_bytes;   // input plane, Veff / Prev tile, whole stage (128-B multiples)
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -77,39 +80,61 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
         "r"(parity)
         : "memory");
 }
-__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *tmap, uint64_t *bar, int x, int y, int z, int c)
+__device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ double2 lds2(uint32_t addr)
+{
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap *tmap, uint64_t *bar, int x, int y, int z, int c)
 {
     asm volatile(
         "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(
-            smem_u32(dst)),
+            dst),
         "l"(tmap), "r"(x), "r"(y), "r"(z), "r"(c), "r"(smem_u32(bar))
         : "memory");
 }
-__device__ __forceinline__ double2 ldg_stream(const double *p)
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *tmap, uint64_t *bar, int x, int y, int z)
 {
-    double2 v;
-    asm volatile("ld.global.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
-    return v;
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+            dst),
+        "l"(tmap), "r"(x), "r"(y), "r"(z), "r"(smem_u32(bar))
+        : "memory");
 }
 
-template <int AY, bool HAS_PREV>
-__global__ void __launch_bounds__(AY == 2 ? 384 : 288, 1)
-stencil_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ TmaParams P)
+// AY: rows per consumer thread (2: 4 points / 168 registers, 1: 2 points / ~100 registers, twice the warps);
+// CW, CNX: compile-time smem pitches (doubles) of the input plane and of the Veff / Prev tiles, 0 = run time (P.W, P.nx).
+template <int AY, int CW, int CNX, bool HAS_PREV>
+__global__ void __launch_bounds__(AY == 1 ? MAX_THREADS_AY1 : MAX_THREADS_AY2, AY == 1 ? 2 : 1)
+stencil_tma_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_constant__ CUtensorMap tmap_v,
+                   const __grid_constant__ CUtensorMap tmap_p, const __grid_constant__ TmaParams P)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    uint64_t *bar_full = reinterpret_cast<uint64_t *>(smem_raw);   // [NSTAGE] TMA landed
-    uint64_t *bar_ready = bar_full + NSTAGE;                       // [NSTAGE] halo patched, consumers may read
-    uint64_t *bar_empty = bar_ready + NSTAGE;                      // [NSTAGE] consumers done
-    unsigned char *stages = smem_raw + 256;
-    const int rows = P.TY + 2 * R;
-    const uint32_t stage_bytes = (uint32_t)(P.W * rows * 8);
+    // barriers first, stages after them at the next 128-byte boundary (TMA destination alignment)
+    uint64_t *bar_full = reinterpret_cast<uint64_t *>(smem_raw);    // [MAX_STAGES] TMA landed
+    uint64_t *bar_empty = bar_full + MAX_STAGES;                    // [MAX_STAGES] consumers done
+    const uint32_t stage0 = (smem_u32(smem_raw) + 2 * MAX_STAGES * 8 + 127u) & ~127u;
 
     const int tid = threadIdx.x;
     const int n_cwarps = (P.n_consumers + 31) >> 5;
     if (tid == 0) {
-        for (int s = 0; s < NSTAGE; ++s) {
+        for (int s = 0; s < P.nstage; ++s) {
             mbar_init(&bar_full[s], 1);
-            mbar_init(&bar_ready[s], 1);
             mbar_init(&bar_empty[s], (uint32_t)n_cwarps);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -127,50 +152,38 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_consta
     const int z1 = min(z0 + P.zchunk_len, P.nz);
     const int nzc = z1 - z0;
     const int nsteps = nzc + 2 * R;          // input planes z0-6 .. z1+5
+    const int W = CW ? CW : P.W;
+    const int NX = CNX ? CNX : P.nx;
 
     if (tid < 32) {
-        // ================================ producer warp ================================================
-        const int lane = tid;
-        const int nboxes = rows / BOX_ROWS;
-        auto issue_plane = [&](int s) {
-            const int stage = s % NSTAGE;
+        // ================================ producer warp (one lane) =======================================
+        if (tid != 0) return;
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_x) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_v) : "memory");
+        if (HAS_PREV) asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_p) : "memory");
+        const int nboxes = (P.TY + 2 * R) / BOX_ROWS;
+        const uint32_t box_bytes = (uint32_t)(BOX_ROWS * W * 8);
+        const uint32_t tile_tx = (uint32_t)(P.TY * NX * 8);
+        int stage = 0;
+        uint32_t phase = 0;
+        for (int s = 0; s < nsteps; ++s) {
+            if (s >= P.nstage) {
+                while (!mbar_try_wait(&bar_empty[stage], phase ^ 1u)) __nanosleep(40);   // do not steal issue slots
+            }
+            const bool do_xy = (s >= R) && (s < R + nzc);
+            const bool do_prev = HAS_PREV && (s >= 2 * R);
             int zin = z0 - R + s;
             if (P.per_z) { if (zin < 0) zin += P.nz; else if (zin >= P.nz) zin -= P.nz; }
-            unsigned char *dst = stages + (size_t)stage * stage_bytes;
-            mbar_arrive_expect_tx(&bar_full[stage], stage_bytes);
+            const uint32_t dst = stage0 + (uint32_t)stage * P.stage_bytes;
+            mbar_arrive_expect_tx(&bar_full[stage], P.psi_bytes + (do_xy ? tile_tx : 0u) + (do_prev ? tile_tx : 0u));
             for (int b = 0; b < nboxes; ++b) {
                 int y = y0 - R + b * BOX_ROWS;
                 if (P.per_y) { if (y < 0) y += P.ny; else if (y >= P.ny) y -= P.ny; }
-                tma_load_4d(dst + (size_t)b * BOX_ROWS * P.W * 8, &tmap, &bar_full[stage], -R, y, zin, col);
+                tma_load_4d(dst + (uint32_t)b * box_bytes, &tmap_x, &bar_full[stage], P.x_start, y, zin, col);
             }
-        };
-        if (lane == 0) {
-            asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap) : "memory");
-            for (int s = 0; s < NSTAGE - LAG && s < nsteps; ++s) issue_plane(s);
-        }
-        for (int i = 0; i < nsteps; ++i) {
-            const int snew = i + NSTAGE - LAG;
-            if (snew < nsteps && lane == 0) {
-                if (i >= LAG) {
-                    const int sold = i - LAG;    // plane that used the stage before
-                    mbar_wait(&bar_empty[sold % NSTAGE], (uint32_t)((sold / NSTAGE) & 1));
-                }
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                issue_plane(snew);
-            }
-            const int stage = i % NSTAGE;
-            mbar_wait(&bar_full[stage], (uint32_t)((i / NSTAGE) & 1));
-            if (P.per_x) {
-                double *pl = reinterpret_cast<double *>(stages + (size_t)stage * stage_bytes);
-                for (int k = lane; k < rows * 2 * R; k += 32) {
-                    const int r = k / (2 * R), j = k - r * (2 * R);
-                    double *row = pl + r * P.W;
-                    if (j < R) row[j] = row[j + P.nx];                 // left halo  <- last 6 of the row
-                    else row[P.nx + j] = row[j];                       // right halo <- first 6 (j in 6..11 -> sx nx+6..nx+11)
-                }
-            }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&bar_ready[stage]);
+            if (do_xy) tma_load_3d(dst + P.psi_bytes, &tmap_v, &bar_full[stage], 0, y0, z0 - R + s);
+            if (do_prev) tma_load_4d(dst + P.psi_bytes + P.tile_bytes, &tmap_p, &bar_full[stage], 0, y0, z0 - 2 * R + s, col);
+            if (++stage == P.nstage) { stage = 0; phase ^= 1u; }
         }
         return;
     }
@@ -181,14 +194,22 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_consta
     const int cta = active ? ct : 0;                 // inactive lanes shadow thread 0 and never store
     const int ty = cta / P.ntx, tx = cta - ty * P.ntx;
     const int lane = tid & 31;
-    const int pitchB = P.W * 8;
-    // byte offset of the thread's first own point inside a stage: row (ty*AY + 6), column (2*tx + 6)
-    const uint32_t thr_off = (uint32_t)(((ty * AY + R) * P.W + 2 * tx + R) * 8);
+    const uint32_t pitchB = (uint32_t)W * 8u;
+    const uint32_t tile_pitchB = (uint32_t)NX * 8u;
+    // shared-memory byte addresses (relative to the stage) of the x-neighbour pairs tx-3 .. tx+3 in the first own
+    // row; a periodic x axis wraps the pair index instead of storing halo columns
+    uint32_t xo[7];
+#pragma unroll
+    for (int k = 0; k < 7; ++k) {
+        int p = tx + k - 3;
+        if (P.per_x) { if (p < 0) p += P.ntx; else if (p >= P.ntx) p -= P.ntx; }
+        else p += 3;
+        xo[k] = (uint32_t)(ty * AY + R) * pitchB + (uint32_t)p * 16u;
+    }
+    const uint32_t tile_off = P.psi_bytes + (uint32_t)((ty * AY * NX + 2 * tx) * 8);   // own pair inside the Veff tile
     const int64_t plane = (int64_t)P.nx * P.ny;
-    const int64_t pt_off = (int64_t)(y0 + ty * AY) * P.nx + 2 * tx;     // offset of the own point inside a plane
-    const double *veff_p = P.veff + pt_off;
-    double *out_p = P.out + (int64_t)col * P.ldo + pt_off;
-    const double *prev_p = HAS_PREV ? P.prev + (int64_t)col * P.ldp + pt_off : nullptr;
+    // running output pointer: plane z0 - 12 at step 0, advanced by one plane per step
+    double *out_z = P.out + (int64_t)col * P.ldo + (int64_t)(y0 + ty * AY) * P.nx + 2 * tx + (int64_t)(z0 - 2 * R) * plane;
 
     double acc[NSLOT][AY][2];
 #pragma unroll
@@ -196,35 +217,20 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_consta
 #pragma unroll
         for (int a = 0; a < AY; ++a) acc[s][a][0] = acc[s][a][1] = 0.0;
 
-    int s = 0;
+    int s = 0, stage = 0;
+    uint32_t phase = 0;
     for (int sb = 0; sb < nsteps; sb += NSLOT) {
 #pragma unroll
         for (int ph = 0; ph < NSLOT; ++ph) {
             if (s >= nsteps) break;
-            const int stage = s % NSTAGE;
-            const int zin = z0 - R + s;              // plane arriving (unwrapped index)
-            const int zo = zin - R;                  // plane completed by this step
             const bool do_xy = (s >= R) && (s < R + nzc);
             const bool do_store = (s >= 2 * R);
+            const uint32_t st = stage0 + (uint32_t)stage * P.stage_bytes;
 
-            // early global loads for this step
-            double2 pv[AY], vf[AY];
-            if (HAS_PREV && do_store) {
-#pragma unroll
-                for (int a = 0; a < AY; ++a) pv[a] = ldg_stream(prev_p + (int64_t)zo * plane + a * P.nx);
-            }
-            if (do_xy) {
-#pragma unroll
-                for (int a = 0; a < AY; ++a)
-                    vf[a] = *reinterpret_cast<const double2 *>(veff_p + (int64_t)zin * plane + a * P.nx);
-            }
-
-            mbar_wait(&bar_ready[stage], (uint32_t)((s / NSTAGE) & 1));
-            const unsigned char *sp = stages + (size_t)stage * stage_bytes + thr_off;
-#define LD2(ptr) (*reinterpret_cast<const double2 *>(ptr))
+            mbar_wait(&bar_full[stage], phase);
             double2 own[AY];
 #pragma unroll
-            for (int a = 0; a < AY; ++a) own[a] = LD2(sp + a * pitchB);
+            for (int a = 0; a < AY; ++a) own[a] = lds2(st + xo[3] + a * pitchB);
 
             // ---- z taps: this plane feeds the 12 neighbouring output planes --------------------------------
 #pragma unroll
@@ -248,44 +254,58 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_consta
             if (do_xy) {
 #pragma unroll
                 for (int a = 0; a < AY; ++a) {
-                    const unsigned char *rp = sp + a * pitchB;
-                    double h[2 * R + 2];       // x - 6 .. x + 7
-                    {
-                        const double2 m3 = LD2(rp - 48), m2 = LD2(rp - 32), m1 = LD2(rp - 16);
-                        const double2 p1 = LD2(rp + 16), p2 = LD2(rp + 32), p3 = LD2(rp + 48);
-                        h[0] = m3.x; h[1] = m3.y; h[2] = m2.x; h[3] = m2.y; h[4] = m1.x; h[5] = m1.y;
-                        h[6] = own[a].x; h[7] = own[a].y;
-                        h[8] = p1.x; h[9] = p1.y; h[10] = p2.x; h[11] = p2.y; h[12] = p3.x; h[13] = p3.y;
-                    }
-                    double s0 = fma(P.alpha, vf[a].x, P.c0a) * own[a].x;
-                    double s1 = fma(P.alpha, vf[a].y, P.c0a) * own[a].y;
-#pragma unroll
-                    for (int p = 1; p <= R; ++p) {
-                        s0 = fma(P.cx[p], h[6 - p], s0);
-                        s0 = fma(P.cx[p], h[6 + p], s0);
-                        s1 = fma(P.cx[p], h[7 - p], s1);
-                        s1 = fma(P.cx[p], h[7 + p], s1);
-                    }
-                    acc[ph][a][0] += s0;
-                    acc[ph][a][1] += s1;
+                    const double2 vf = lds2(st + tile_off + a * tile_pitchB);
+                    const double2 m3 = lds2(st + xo[0] + a * pitchB), m2 = lds2(st + xo[1] + a * pitchB);
+                    const double2 m1 = lds2(st + xo[2] + a * pitchB), p1 = lds2(st + xo[4] + a * pitchB);
+                    const double2 p2 = lds2(st + xo[5] + a * pitchB), p3 = lds2(st + xo[6] + a * pitchB);
+                    // left and right halves are separate dependency chains
+                    double l0 = fma(P.alpha, vf.x, P.c0a) * own[a].x;
+                    double l1 = fma(P.alpha, vf.y, P.c0a) * own[a].y;
+                    double r0 = P.cx[1] * own[a].y, r1 = P.cx[1] * own[a].x;   // x+1 of point 0, x-1 of point 1
+                    l0 = fma(P.cx[1], m1.y, l0); l0 = fma(P.cx[2], m1.x, l0); l0 = fma(P.cx[3], m2.y, l0);
+                    l0 = fma(P.cx[4], m2.x, l0); l0 = fma(P.cx[5], m3.y, l0); l0 = fma(P.cx[6], m3.x, l0);
+                    r0 = fma(P.cx[2], p1.x, r0); r0 = fma(P.cx[3], p1.y, r0); r0 = fma(P.cx[4], p2.x, r0);
+                    r0 = fma(P.cx[5], p2.y, r0); r0 = fma(P.cx[6], p3.x, r0);
+                    r1 = fma(P.cx[2], m1.y, r1); r1 = fma(P.cx[3], m1.x, r1); r1 = fma(P.cx[4], m2.y, r1);
+                    r1 = fma(P.cx[5], m2.x, r1); r1 = fma(P.cx[6], m3.y, r1);
+                    l1 = fma(P.cx[1], p1.x, l1); l1 = fma(P.cx[2], p1.y, l1); l1 = fma(P.cx[3], p2.x, l1);
+                    l1 = fma(P.cx[4], p2.y, l1); l1 = fma(P.cx[5], p3.x, l1); l1 = fma(P.cx[6], p3.y, l1);
+                    acc[ph][a][0] += l0 + r0;
+                    acc[ph][a][1] += l1 + r1;
                 }
+                double ys[AY][2];
+#pragma unroll
+                for (int a = 0; a < AY; ++a) ys[a][0] = ys[a][1] = 0.0;
 #pragma unroll
                 for (int rr = -R; rr < AY + R; ++rr) {
-                    const double2 yv = (rr >= 0 && rr < AY) ? own[rr >= 0 && rr < AY ? rr : 0] : LD2(sp + rr * pitchB);
+                    const double2 yv = (rr >= 0 && rr < AY) ? own[rr >= 0 && rr < AY ? rr : 0]
+                                                            : lds2(st + xo[3] + rr * (int)pitchB);
 #pragma unroll
                     for (int a = 0; a < AY; ++a) {
                         const int dist = rr > a ? rr - a : a - rr;
                         if (dist >= 1 && dist <= R) {
-                            acc[ph][a][0] = fma(P.cy[dist], yv.x, acc[ph][a][0]);
-                            acc[ph][a][1] = fma(P.cy[dist], yv.y, acc[ph][a][1]);
+                            if (rr < a) {      // lower rows go to the side chain, upper rows to the accumulator
+                                ys[a][0] = fma(P.cy[dist], yv.x, ys[a][0]);
+                                ys[a][1] = fma(P.cy[dist], yv.y, ys[a][1]);
+                            } else {
+                                acc[ph][a][0] = fma(P.cy[dist], yv.x, acc[ph][a][0]);
+                                acc[ph][a][1] = fma(P.cy[dist], yv.y, acc[ph][a][1]);
+                            }
                         }
                     }
                 }
+#pragma unroll
+                for (int a = 0; a < AY; ++a) { acc[ph][a][0] += ys[a][0]; acc[ph][a][1] += ys[a][1]; }
             }
-#undef LD2
+            double2 pv[AY];
+            if (HAS_PREV && do_store) {
+#pragma unroll
+                for (int a = 0; a < AY; ++a) pv[a] = lds2(st + tile_off + P.tile_bytes + a * tile_pitchB);
+            }
             // ---- this stage is free again ---------------------------------------------------------------------
             __syncwarp();
             if (lane == 0) mbar_arrive(&bar_empty[stage]);
+            if (++stage == P.nstage) { stage = 0; phase ^= 1u; }
 
             // ---- output plane zo has all 37 taps: recurrence axpy + store --------------------------------------
             if (do_store) {
@@ -301,34 +321,106 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_consta
                             o.x = acc[cs][a][0];
                             o.y = acc[cs][a][1];
                         }
-                        *reinterpret_cast<double2 *>(out_p + (int64_t)zo * plane + a * P.nx) = o;
+                        *reinterpret_cast<double2 *>(out_z + a * NX) = o;
                     }
                 }
             }
+            out_z += plane;
             ++s;
         }
     }
 }
 
-struct TileChoice { int TY, AY; };
+struct TileChoice { int AY, TY, threads, ctas_per_sm, nstage, W, variant; uint32_t psi_bytes, tile_bytes, stage_bytes; size_t smem; };
 
-// tile rows: a multiple of 6 dividing ny, as tall as the register budget allows (consumers <= cap)
-bool choose_tile(int nx, int ny, TileChoice *tc)
+constexpr int SMEM_PER_SM = 227 * 1024;
+
+typedef void (*StencilKernel)(const CUtensorMap, const CUtensorMap, const CUtensorMap, const TmaParams);
+
+// compile-time pitch variants: (input-plane pitch W, tile pitch nx); variant 0 is the run-time-pitch kernel
+constexpr int N_VARIANTS = 4;
+constexpr int VAR_W[N_VARIANTS] = {0, 48, 64, 96};
+constexpr int VAR_NX[N_VARIANTS] = {0, 48, 60, 96};
+
+template <int AYV, bool HP>
+StencilKernel pick_variant(int v)
 {
-    const int ntx = nx / 2;
-    int best_ty = 0, best_ay = 0;
-    for (int ay = 2; ay <= 2; ++ay) {     // AY = 3 spills at the 224-register cap: not instantiated
-        const int cap = (ay == 2) ? 352 : 256;
-        for (int ty = ny; ty >= 6; --ty) {
-            if (ny % ty || ty % BOX_ROWS || ty % ay) continue;
-            if (ntx * (ty / ay) > cap) continue;
-            if (ty > best_ty) { best_ty = ty; best_ay = ay; }
-            break;
-        }
+    switch (v) {
+    case 1: return stencil_tma_kernel<AYV, VAR_W[1], VAR_NX[1], HP>;
+    case 2: return stencil_tma_kernel<AYV, VAR_W[2], VAR_NX[2], HP>;
+    case 3: return stencil_tma_kernel<AYV, VAR_W[3], VAR_NX[3], HP>;
+    default: return stencil_tma_kernel<AYV, 0, 0, HP>;
     }
-    if (!best_ty) return false;
-    tc->TY = best_ty; tc->AY = best_ay;
-    return true;
+}
+
+StencilKernel pick_kernel(int ay, int variant, bool has_prev)
+{
+    if (ay == 1) return has_prev ? pick_variant<1, true>(variant) : pick_variant<1, false>(variant);
+    return has_prev ? pick_variant<2, true>(variant) : pick_variant<2, false>(variant);
+}
+
+// Tile rows TY: a multiple of 6 (TMA box rows) and of AY dividing ny.  Preference: the tallest tile whose CTA still
+// fits at least twice on an SM (the kernels are register-limited), else the smallest valid tile.  The ring depth is
+// whatever the per-CTA share of shared memory allows.
+bool choose_tile(const sparc_gpu_ctx *ctx, TileChoice *tc)
+{
+    const int nx = ctx->n[0], ny = ctx->n[1];
+    const int ntx = nx / 2;
+    const bool per_x = ctx->bc[0] == 0;
+    const int ay = ctx->opt_stencil_ay == 1 ? 1 : 2;
+    const int max_threads = ay == 1 ? MAX_THREADS_AY1 : MAX_THREADS_AY2;
+    const int max_warps_sm = ay == 1 ? 21 : 12;                       // 65536 / (regs per thread * 32)
+    // candidates: maximise the consumer threads resident per SM; among near-ties take the smallest tile with a halo
+    // factor (TY + 12) / TY <= 2 (more CTAs per SM, shorter tail), else the tallest (measured, profiles/)
+    int ty = 0, best_useful = 0;
+    for (int pass = 0; pass < 2; ++pass) {
+        int pick_small = 0, pick_large = 0;
+        for (int t = BOX_ROWS; t <= ny; t += BOX_ROWS) {
+            if (ny % t || t % ay) continue;
+            if (ctx->opt_stencil_ty > 0 && t != ctx->opt_stencil_ty) continue;
+            const int cons = ntx * (t / ay);
+            const int threads = 32 + (cons + 31) / 32 * 32;
+            if (threads > max_threads) continue;
+            const int useful = std::max(1, max_warps_sm / (threads / 32)) * cons;
+            if (pass == 0) { best_useful = std::max(best_useful, useful); continue; }
+            if (useful * 20 < best_useful * 19) continue;
+            if (t >= 2 * R && !pick_small) pick_small = t;
+            pick_large = t;
+        }
+        if (pass == 1) ty = pick_small ? pick_small : pick_large;
+    }
+    if (!ty) return false;
+    tc->AY = ay;
+    tc->TY = ty;
+    tc->threads = 32 + (ntx * (ty / ay) + 31) / 32 * 32;
+    tc->W = (int)round_up_i64(per_x ? nx : nx + 2 * R, 8);
+    tc->variant = 0;
+    for (int v = 1; v < N_VARIANTS; ++v)
+        if (VAR_W[v] == tc->W && VAR_NX[v] == nx) tc->variant = v;
+    tc->psi_bytes = (uint32_t)(tc->W * (ty + 2 * R) * 8);
+    tc->tile_bytes = (uint32_t)round_up_i64((int64_t)ty * nx * 8, 128);
+    tc->stage_bytes = tc->psi_bytes + 2 * tc->tile_bytes;
+    StencilKernel kern = pick_kernel(ay, tc->variant, true);
+    for (int ctas = 5; ctas >= 1; --ctas) {
+        const int64_t budget = SMEM_PER_SM / ctas - 1024 - 512;
+        int nstage = (int)std::min<int64_t>(MAX_STAGES, budget / tc->stage_bytes);
+        nstage = std::min(nstage, ctx->opt_stencil_stages > 0 ? ctx->opt_stencil_stages : 3);   // deeper rings measured slower
+        if (nstage < 2 || (nstage < 3 && ctas > 1)) continue;
+        const size_t smem = 512 + (size_t)nstage * tc->stage_bytes;
+        int occ = 0;
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, tc->threads, smem) != cudaSuccess) {
+            (void)cudaGetLastError();
+            continue;
+        }
+        if (occ < ctas && ctas > 1) continue;
+        if (occ < 1) continue;
+        tc->nstage = nstage;
+        tc->ctas_per_sm = std::min(occ, ctas);
+        tc->smem = smem;
+        return true;
+    }
+    return false;
 }
 
 bool a16(const void *p) { return ((uintptr_t)p & 15) == 0; }
@@ -336,6 +428,22 @@ bool a16(const void *p) { return ((uintptr_t)p & 15) == 0; }
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// (x, y, z[, column]) tensor map over an N_d x ncols column-major block; box = bx x by x 1 [x 1]
+bool encode_map(const sparc_gpu_ctx *ctx, CUtensorMap *tm, const void *base, int rank, int64_t ncols, int64_t ld, int bx,
+                int by)
+{
+    const int nx = ctx->n[0], ny = ctx->n[1], nz = ctx->n[2];
+    const cuuint64_t gdim[4] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nz, (cuuint64_t)std::max<int64_t>(ncols, 1)};
+    const cuuint64_t gstr[3] = {(cuuint64_t)nx * 8, (cuuint64_t)nx * ny * 8, (cuuint64_t)ld * 8};
+    const cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, 1, 1};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult cr = ((EncodeTiledFn)ctx->fn_encode_tiled)(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, (cuuint32_t)rank, (void *)base,
+                                                        gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                                        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                                                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return cr == CUDA_SUCCESS;
+}
 
 }  // namespace
 
@@ -349,7 +457,7 @@ bool stencil_tma_supported(const sparc_gpu_ctx *ctx, const double *X, int64_t ld
     if (ny % BOX_ROWS) return false;
     if (!a16(X) || !a16(Out) || (Prev && !a16(Prev)) || (ldx & 1) || (ldo & 1) || (Prev && (ldp & 1))) return false;
     TileChoice tc;
-    return choose_tile(nx, ny, &tc);
+    return choose_tile(ctx, &tc);
 }
 
 int launch_stencil_tma(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double *Out, int64_t ldo, const double *Prev,
@@ -359,62 +467,51 @@ int launch_stencil_tma(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double 
     if (!stencil_tma_supported(ctx, X, ldx, Out, ldo, has_prev ? Prev : nullptr, ldp)) return SPARC_GPU_UNSUPPORTED;
     const int nx = ctx->n[0], ny = ctx->n[1], nz = ctx->n[2];
     TileChoice tc;
-    choose_tile(nx, ny, &tc);
+    choose_tile(ctx, &tc);
 
     TmaParams P;
     for (int p = 0; p <= R; ++p) { P.cx[p] = alpha * ctx->coef.cx[p]; P.cy[p] = alpha * ctx->coef.cy[p]; P.cz[p] = alpha * ctx->coef.cz[p]; }
     P.c0a = alpha * (ctx->coef.c0 + shift);
     P.alpha = alpha; P.beta = beta;
-    P.veff = ctx->d_veff;
-    P.ldo = ldo; P.ldp = ldp;
+    P.ldo = ldo;
     P.nx = nx; P.ny = ny; P.nz = nz;
-    P.W = (int)round_up_i64(nx + 2 * R, 8);
+    P.per_x = ctx->bc[0] == 0; P.per_y = ctx->bc[1] == 0; P.per_z = ctx->bc[2] == 0;
+    P.W = tc.W;
+    P.x_start = P.per_x ? 0 : -R;
     P.TY = tc.TY;
     P.ntx = nx / 2;
     P.n_consumers = P.ntx * (tc.TY / tc.AY);
+    P.nstage = tc.nstage;
     P.ytiles = ny / tc.TY;
-    P.per_x = ctx->bc[0] == 0; P.per_y = ctx->bc[1] == 0; P.per_z = ctx->bc[2] == 0;
+    P.psi_bytes = tc.psi_bytes; P.tile_bytes = tc.tile_bytes; P.stage_bytes = tc.stage_bytes;
 
-    const int threads = 32 + (P.n_consumers + 31) / 32 * 32;
-    const size_t smem = 256 + (size_t)NSTAGE * P.W * (tc.TY + 2 * R) * 8;
-    if (smem > 227 * 1024) return SPARC_GPU_UNSUPPORTED;
+    CUtensorMap tmap_v;
+    if (!encode_map(ctx, &tmap_v, ctx->d_veff, 3, 1, ctx->nd, nx, tc.TY)) return SPARC_GPU_CUDA_ERROR;
+    StencilKernel kern = pick_kernel(tc.AY, tc.variant, has_prev);
+    SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc.smem));
 
-    // z chunks: split the march only as far as needed to give the chip about two waves of CTAs
     const int64_t max_cols_per_launch = std::max<int64_t>(1, (int64_t)INT32_MAX / ((int64_t)P.ytiles * nz));
     for (int64_t j0 = 0; j0 < ncols; j0 += max_cols_per_launch) {
         const int64_t nb = std::min<int64_t>(max_cols_per_launch, ncols - j0);
+        // z chunks: split the march only as far as needed to give the chip about two waves of CTAs
         int zchunks = 1;
         const int64_t base = nb * P.ytiles;
-        const int64_t want = 2LL * ctx->sm_count;
+        const int64_t want = 2LL * ctx->sm_count * tc.ctas_per_sm;
         if (base < want) zchunks = (int)std::min<int64_t>((want + base - 1) / base, std::max(1, nz / 12));
+        if (ctx->opt_stencil_zchunks > 0) zchunks = std::min(ctx->opt_stencil_zchunks, nz);
         P.zchunk_len = (nz + zchunks - 1) / zchunks;
         P.zchunks = (nz + P.zchunk_len - 1) / P.zchunk_len;
         P.out = Out + j0 * ldo;
-        P.prev = has_prev ? Prev + j0 * ldp : nullptr;
 
-        CUtensorMap tmap;
-        const cuuint64_t gdim[4] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nz, (cuuint64_t)nb};
-        const cuuint64_t gstr[3] = {(cuuint64_t)nx * 8, (cuuint64_t)nx * ny * 8, (cuuint64_t)ldx * 8};
-        const cuuint32_t box[4] = {(cuuint32_t)P.W, BOX_ROWS, 1, 1};
-        const cuuint32_t estr[4] = {1, 1, 1, 1};
-        CUresult cr = ((EncodeTiledFn)ctx->fn_encode_tiled)(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4,
-                                                            (void *)(X + j0 * ldx), gdim, gstr, box, estr,
-                                                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                                                            CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                                                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (cr != CUDA_SUCCESS) return SPARC_GPU_CUDA_ERROR;
+        CUtensorMap tmap_x, tmap_p;
+        if (!encode_map(ctx, &tmap_x, X + j0 * ldx, 4, nb, ldx, tc.W, BOX_ROWS)) return SPARC_GPU_CUDA_ERROR;
+        if (!encode_map(ctx, &tmap_p, has_prev ? Prev + j0 * ldp : X + j0 * ldx, 4, nb, has_prev ? ldp : ldx, nx, tc.TY))
+            return SPARC_GPU_CUDA_ERROR;
 
         const unsigned grid = (unsigned)(nb * P.ytiles * P.zchunks);
-#define LAUNCH_TMA(AYV, HP)                                                                                          \
-        do {                                                                                                         \
-            auto kern = stencil_tma_kernel<AYV, HP>;                                                                 \
-            SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));      \
-            prof_begin(ctx, KK_STENCIL_TMA, st);                                                                     \
-            kern<<<grid, threads, smem, st>>>(tmap, P);                                                              \
-            prof_end(ctx, KK_STENCIL_TMA, st);                                                                       \
-        } while (0)
-        if (has_prev) LAUNCH_TMA(2, true); else LAUNCH_TMA(2, false);
-#undef LAUNCH_TMA
+        prof_begin(ctx, KK_STENCIL_TMA, st);
+        kern<<<grid, tc.threads, tc.smem, st>>>(tmap_x, tmap_v, tmap_p, P);
+        prof_end(ctx, KK_STENCIL_TMA, st);
     }
     SPARC_CUDA_TRY(cudaGetLastError());
     return SPARC_GPU_SUCCESS;

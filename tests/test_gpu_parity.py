@@ -99,6 +99,30 @@ def test_h_apply_and_filter_small(torch, api, wl, path):
     g.close()
 
 
+@pytest.mark.parametrize("mode", [0, 1])
+def test_nonlocal_modes(torch, api, mode):
+    """Both nonlocal paths (0: fused per-atom kernel with atomic scatter, 1: project + pull, deterministic) against
+    the oracle, on heavily overlapping supports, a ragged number of columns and more rows than one shared tile."""
+    pos = np.array([[3.0, 3.1, 3.3], [3.6, 3.0, 2.9], [2.5, 3.4, 3.8], [6.1, 0.2, 0.7], [0.1, 6.0, 6.2]])
+    wl = wlmod.make_custom("nlmodes", (24, 18, 20), (0.3, 0.32, 0.31), (0, 0, 1), 37, 3, pos, [9, 4, 1, 9, 9], 2.4,
+                           seed=21)
+    assert max(np.diff(wl.supp_ptr)) > 512          # several shared-memory tiles per atom
+    g = api.SparcGpu(wl)
+    g.set_option("nonlocal_mode", mode)
+    X = wl.psi_columns(range(wl.ns))
+    H = orc.Hamiltonian(wl)
+    Yg = g.hamiltonian_apply(api.colmajor_from_numpy(X))
+    check_col(api.colmajor_to_numpy(Yg), H.apply(X), f"nonlocal_mode {mode} H*Psi")
+    Pg = api.colmajor_from_numpy(X)
+    g.chebyshev_filter(Pg, 3, wl.a, wl.b, wl.a0, col_block=17)
+    check_col(api.colmajor_to_numpy(Pg), H.chebyshev_filter(X, 3, wl.a, wl.b, wl.a0), f"nonlocal_mode {mode} filter")
+    if mode == 1:       # the pull path is bitwise reproducible
+        P2 = api.colmajor_from_numpy(X)
+        g.chebyshev_filter(P2, 3, wl.a, wl.b, wl.a0, col_block=17)
+        assert torch.equal(P2, Pg)
+    g.close()
+
+
 @pytest.mark.parametrize("fd_order", [2, 4, 6, 8, 10])
 def test_lower_fd_orders(torch, api, fd_order):
     pos = np.array([[1.0, 2.0, 3.0]])
