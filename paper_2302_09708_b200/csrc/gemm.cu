@@ -181,18 +181,28 @@ gemm_simple_kernel(const double *__restrict__ A, int64_t lda, const double *__re
 
 struct SplitPlan { int splits; int64_t k_chunk; };
 
+// Split-K plan for the tall contraction (K = N_d >> M, N): the number of CTAs (tiles x splits) is chosen as the
+// nearest-to-whole number of waves over the SMs (one CTA per SM), preferring few splits; partial products go to the
+// workspace and are summed in a fixed order (deterministic).
 SplitPlan plan_tn(const sparc_gpu_ctx *ctx, int64_t M, int64_t N, int64_t K)
 {
     const int64_t tiles = ((M + BM - 1) / BM) * ((N + BN - 1) / BN);
-    int64_t splits = 1;
-    if (tiles < (int64_t)ctx->sm_count) {
-        splits = (2 * (int64_t)ctx->sm_count + tiles - 1) / tiles;
-        const int64_t max_splits = std::max<int64_t>(1, K / (8 * BK));
-        splits = std::max<int64_t>(1, std::min(splits, max_splits));
+    const int64_t sms = std::max(1, ctx->sm_count);
+    const int64_t max_splits = std::max<int64_t>(1, std::min<int64_t>(64, K / (16 * BK)));
+    const int64_t ws_cap = (int64_t)2 << 30;                       // at most 2 GiB of partial products
+    int64_t best_s = 1;
+    double best_cost = 1e300;
+    for (int64_t s = 1; s <= max_splits; ++s) {
+        if (s > 1 && s * M * N * 8 > ws_cap) break;
+        const int64_t ctas = tiles * s;
+        const int64_t waves = (ctas + sms - 1) / sms;
+        // time ~ waves * (K / s) per CTA, plus the reduction traffic (s partials of M x N) relative to the main loop
+        const double cost = (double)waves * ((double)K / (double)s + 64.0) + (s > 1 ? 0.02 * (double)s * (double)K / 64.0 / (double)std::max<int64_t>(1, tiles / 8 + 1) : 0.0);
+        if (cost < best_cost * 0.995) { best_cost = cost; best_s = s; }
     }
-    int64_t chunk = (K + splits - 1) / splits;
+    int64_t chunk = (K + best_s - 1) / best_s;
     chunk = round_up_i64(std::max<int64_t>(chunk, 1), BK);
-    splits = (K + chunk - 1) / chunk;
+    int64_t splits = (K + chunk - 1) / chunk;
     if (splits < 1) splits = 1;
     return {(int)splits, chunk};
 }
