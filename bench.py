@@ -241,7 +241,7 @@ def run_ours(args):
     # ---- roofline of the dominant kernel: per-launch CUDA events inside the library, same launch config ------
     roofline = None
     kinds = {0: "stencil_generic", 1: "stencil_tma", 2: "nl_project", 3: "nl_pull", 4: "gemm_tn", 5: "gemm_nn",
-             6: "splitk_reduce", 7: "copy2d"}
+             6: "splitk_reduce", 7: "copy2d", 8: "nl_fused"}
     share = {}
     if rank == 0:
         g.set_option("profile_reset", 1)
