@@ -126,6 +126,14 @@ int sparc_gpu_rotate(sparc_gpu_ctx *ctx, double *Psi_dev, int64_t ld, int64_t ns
 int sparc_gpu_fill_uniform(double *dst_dev, int64_t count, uint64_t seed, uint64_t stream_id,
                            uint64_t index0, double lo, double hi, int device, void *stream);
 
+/* Register-resident throughput probes: the roofline denominators of the FP64-bound kernels, measured on the
+ * device the library runs on.  kind 0: FP64 FMA (DFMA) TFLOP/s; kind 1: FP64 tensor
+ * (DMMA m8n8k4) TFLOP/s; kind 2: device copy GB/s (read + write bytes) over scratch_dev.  value_out is a HOST
+ * pointer; scratch_dev a DEVICE buffer of scratch_bytes (>= 64; kind 2 copies its first half onto its second).
+ * Synchronises `stream` (best of 4 timed repetitions after a warm-up).  Not an operator of the method. */
+int sparc_gpu_probe_peak(int device, int kind, double *value_out, void *scratch_dev, int64_t scratch_bytes,
+                         void *stream);
+
 /* Tuning / test knobs.  key: "stencil_path" (0 auto, 1 generic kernel, 2 TMA kernel or UNSUPPORTED),
  * "nonlocal" (1 on, 0 off: drops V_nl, used by closed-form pins), "gemm_path" (0 auto, 1 simple FMA
  * kernel, 2 DMMA kernel).  Unknown key -> INVALID_ARG. */

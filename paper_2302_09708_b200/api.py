@@ -24,7 +24,7 @@ OP_HAMILTONIAN_APPLY, OP_CHEBYSHEV_FILTER, OP_PROJECT, OP_ROTATE = 0, 1, 2, 3
 
 EXPORTS = ["sparc_gpu_create", "sparc_gpu_destroy", "sparc_gpu_set_veff", "sparc_gpu_workspace_bytes",
            "sparc_gpu_hamiltonian_apply", "sparc_gpu_chebyshev_filter", "sparc_gpu_project",
-           "sparc_gpu_rotate", "sparc_gpu_fill_uniform", "sparc_gpu_set_option", "sparc_gpu_get_info",
+           "sparc_gpu_rotate", "sparc_gpu_fill_uniform", "sparc_gpu_set_option", "sparc_gpu_get_info", "sparc_gpu_probe_peak",
            "sparc_gpu_error_string", "sparc_gpu_version"]
 
 
@@ -64,6 +64,7 @@ def load_library(build_if_missing: bool = True):
     lib.sparc_gpu_project.argtypes = [P, P, I64, I64, P, P, I64, P, P]
     lib.sparc_gpu_rotate.argtypes = [P, P, I64, I64, P, I64, P, P]
     lib.sparc_gpu_fill_uniform.argtypes = [P, I64, C.c_uint64, C.c_uint64, C.c_uint64, D, D, I, P]
+    lib.sparc_gpu_probe_peak.argtypes = [I, I, C.POINTER(D), P, I64, P]
     lib.sparc_gpu_set_option.argtypes = [P, C.c_char_p, I64]
     lib.sparc_gpu_get_info.argtypes = [P, C.c_char_p, C.POINTER(I64)]
     lib.sparc_gpu_error_string.argtypes = [I]
@@ -113,6 +114,16 @@ def fill_uniform(t, seed: int, stream_id: int, index0: int, lo: float, hi: float
     _check(load_library().sparc_gpu_fill_uniform(C.c_void_p(t.data_ptr()), t.numel(), seed, stream_id, index0,
                                                  lo, hi, t.device.index or 0, _stream_ptr()), "fill_uniform")
     return t
+
+
+def probe_peak(kind: int, device: int = 0, scratch_bytes: int = 1 << 30) -> float:
+    """kind 0: FP64 FMA TFLOP/s, 1: FP64 DMMA TFLOP/s, 2: device copy GB/s -- measured live (sparc_gpu_probe_peak)."""
+    torch = _torch()
+    scratch = torch.empty(scratch_bytes if kind == 2 else 4096, dtype=torch.uint8, device=f"cuda:{device}")
+    out = C.c_double()
+    _check(load_library().sparc_gpu_probe_peak(int(device), int(kind), C.byref(out), C.c_void_p(scratch.data_ptr()),
+                                               scratch.numel(), _stream_ptr()), "probe_peak")
+    return out.value
 
 
 class SparcGpu:

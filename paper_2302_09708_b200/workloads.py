@@ -138,6 +138,15 @@ class Workload:
     def psi(self) -> np.ndarray:
         return self.psi_columns(range(self.ns))
 
+    def psi_rows(self, rows: Sequence[int]) -> np.ndarray:
+        """Rows `rows` (grid indices) of Psi, all ns columns, as a (len(rows), ns) Fortran-ordered array."""
+        nd = self.nd
+        r = np.asarray(list(rows), dtype=np.uint64)
+        out = np.empty((r.shape[0], self.ns), dtype=np.float64, order="F")
+        for j in range(self.ns):
+            out[:, j] = 2.0 * counter_uniform(self.seed, STREAM_PSI, r + np.uint64(nd * j)) - 1.0
+        return out
+
     def q_matrix(self) -> np.ndarray:
         """Haar-random orthogonal Q (ns x ns, Fortran order): Gaussian matrix -> QR -> sign fix."""
         ns = self.ns

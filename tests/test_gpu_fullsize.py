@@ -1,0 +1,183 @@
+"""Full-size parity for BASELINE.json configs 2-4 in the launch configuration bench.py times (SURVEY.md section 8(c),
+pin P11): the oracle cannot produce 29-82 GB blocks, so it computes SAMPLED outputs one by one --
+
+    filter, H*Psi : a fixed sample of columns (first and last column of every column block + random ones);
+                    columns are independent, so these are exact for the sampled columns;
+    Hs, Ms        : sampled index sets I x J (needs only columns I and J of Psi and of H*Psi);
+    Psi Q         : sampled rows (first / last row of every row panel + random ones), all N_s columns;
+
+plus properties that hold at any size with no oracle at all (P10): rotate(rotate(Psi,Q),Q^T) = Psi,
+||Psi Q||_F = ||Psi||_F, project(rotate(Psi,Q)) = Q^T project(Psi) Q, tr Ms = ||Psi||_F^2, Hs ~ Hs^T.
+All oracle inputs come from the seeded host generator (workloads.py); the device block is produced by the device
+restatement of the same generator (checked bit for bit on the sampled columns / rows)."""
+import math
+import time
+
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from paper_2302_09708_b200 import workloads as wlmod
+
+pytestmark = pytest.mark.gpu
+
+TOL_COL, TOL_FRO = 1e-10, 1e-11          # north_star gates
+TIGHT = 1e-13                            # a correct kernel sits orders below the gate (R16)
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    assert t.cuda.is_available()
+    return t
+
+
+@pytest.fixture(scope="module")
+def api():
+    from paper_2302_09708_b200 import api as a
+    return a
+
+
+def col_err(G, O):
+    return float((np.max(np.abs(G - O), axis=0) / np.linalg.norm(O, axis=0)).max())
+
+
+def fro_err(G, O):
+    return float(np.linalg.norm(G - O) / np.linalg.norm(O))
+
+
+def sample_columns(ns, block, n_random, rng):
+    cols = set()
+    for j0 in range(0, ns, block):
+        cols.add(j0)
+        cols.add(min(j0 + block, ns) - 1)
+    cols.update(int(c) for c in rng.choice(ns, size=min(n_random, ns), replace=False))
+    return sorted(cols)
+
+
+def sample_rows(nd, panel, n_random, rng):
+    rows = set()
+    for r0 in range(0, nd, panel):
+        rows.add(r0)
+        rows.add(min(r0 + panel, nd) - 1)
+    rows.update(int(r) for r in rng.choice(nd, size=n_random, replace=False))
+    return sorted(rows)
+
+
+def fullsize_parity(torch, api, cfg, n_random_cols, n_gram, n_random_rows, check_invariants):
+    t_start = time.time()
+    wl = wlmod.make_workload(cfg)
+    nd, ns, m = wl.nd, wl.ns, wl.degree
+    rng = np.random.default_rng(1000 + cfg)
+    g = api.SparcGpu(wl)
+    H = orc.Hamiltonian(wl)
+    dev = "cuda"
+    col_block = wl.col_block if wl.col_block else min(ns, 1024)      # what bench.py launches
+
+    Psi = torch.empty((ns, nd), dtype=torch.float64, device=dev)
+
+    def refill():
+        api.fill_uniform(Psi, wl.seed, wlmod.STREAM_PSI, 0, -1.0, 1.0)
+
+    refill()
+    cols = sample_columns(ns, col_block, n_random_cols, rng)
+    X = wl.psi_columns(cols)                                          # host generator
+    idx = torch.tensor(cols, device=dev)
+    assert np.array_equal(api.colmajor_to_numpy(Psi[idx]), X), "device fill != host generator"
+    norm2 = float(torch.linalg.vector_norm(Psi)) ** 2
+
+    # ---- H*Psi on the sampled columns -----------------------------------------------------------------------
+    Yg = g.hamiltonian_apply(Psi[idx].contiguous())
+    HX = H.apply(X)
+    e = col_err(api.colmajor_to_numpy(Yg), HX)
+    print(f"[parity] cfg{cfg} H*Psi, {len(cols)} sampled columns: {e:.3e}")
+    assert e <= TOL_COL and e <= TIGHT
+    del Yg
+
+    # ---- Hs, Ms on sampled I x J (raw Psi: every entry needs only columns I, J) -----------------------------
+    Hs, Ms = g.project(Psi, col_block=col_block)
+    I = sorted(set(cols[:n_gram]) | {0, ns - 1})
+    pos = {c: k for k, c in enumerate(cols)}
+    sel = [pos[c] for c in I]
+    Hs_o = orc.gram(X[:, sel], HX[:, sel])
+    Ms_o = orc.gram(X[:, sel], X[:, sel])
+    It = torch.tensor(I, device=dev)
+    Hs_g = Hs[It][:, It].cpu().numpy().T          # tensor [j, i] = M_ij
+    Ms_g = Ms[It][:, It].cpu().numpy().T
+    eh, em = fro_err(Hs_g, Hs_o), fro_err(Ms_g, Ms_o)
+    print(f"[parity] cfg{cfg} Hs / Ms on a sampled {len(I)}x{len(I)} index set: {eh:.3e} / {em:.3e}")
+    assert eh <= TOL_FRO and em <= TOL_FRO and eh <= TIGHT and em <= TIGHT
+    # properties at full size (P10)
+    tr = float(torch.diagonal(Ms).sum())
+    assert abs(tr - norm2) <= 1e-12 * norm2, "tr Ms != ||Psi||_F^2"
+    asym = float(torch.linalg.norm(Hs - Hs.T) / torch.linalg.norm(Hs))
+    print(f"[parity] cfg{cfg} ||Hs - Hs^T||/||Hs|| = {asym:.3e}")
+    assert asym <= 1e-12
+    assert float(torch.linalg.norm(Ms - Ms.T) / torch.linalg.norm(Ms)) <= 1e-12
+
+    # ---- rotation: sampled rows against the oracle, then invariants ------------------------------------------
+    Qn = wl.q_matrix()
+    Q = api.colmajor_from_numpy(Qn)
+    panel = 0                                     # library default, as bench.py
+    rows = sample_rows(nd, max(1, nd // 7), n_random_rows, rng)
+    Xr = wl.psi_rows(rows)
+    R_o = orc.rotate(Xr, Qn)
+    g.rotate(Psi, Q, row_panel=panel)
+    rt = torch.tensor(rows, device=dev)
+    R_g = Psi[:, rt].cpu().numpy().T
+    er = fro_err(R_g, R_o)
+    print(f"[parity] cfg{cfg} Psi*Q on {len(rows)} sampled rows x {ns} columns: {er:.3e}")
+    assert er <= TOL_FRO and er <= TIGHT
+    n2 = float(torch.linalg.vector_norm(Psi)) ** 2
+    assert abs(n2 - norm2) <= 1e-12 * norm2, "||Psi Q||_F != ||Psi||_F"
+    if check_invariants:
+        Hs2, Ms2 = g.project(Psi, col_block=col_block)
+        # tensors hold the transposes (column-major): Q^T Hs Q  <->  Qt^T ... with Qt = Q.T view
+        Qm = Q.T                                  # Qm[i, j] = Q_ij
+        HsR = Qm.T @ Hs.T @ Qm
+        e1 = float(torch.linalg.norm(Hs2.T - HsR) / torch.linalg.norm(HsR))
+        MsR = Qm.T @ Ms.T @ Qm
+        e2 = float(torch.linalg.norm(Ms2.T - MsR) / torch.linalg.norm(MsR))
+        print(f"[parity] cfg{cfg} project(rotate(Psi,Q)) vs Q^T project(Psi) Q: Hs {e1:.3e}, Ms {e2:.3e}")
+        assert e1 <= 1e-11 and e2 <= 1e-11
+        del Hs2, Ms2, HsR, MsR
+    # rotate back with Q^T and compare with the generator on the sampled columns
+    Qt = api.colmajor_from_numpy(np.asfortranarray(Qn.T))
+    g.rotate(Psi, Qt, row_panel=4096)             # a different panel size (R19)
+    back = api.colmajor_to_numpy(Psi[idx])
+    eb = fro_err(back, X)
+    print(f"[parity] cfg{cfg} rotate(rotate(Psi,Q),Q^T) vs Psi on sampled columns: {eb:.3e}")
+    assert eb <= 1e-12
+    del Q, Qt, Hs, Ms
+
+    # ---- the filter, whole block in place, bench.py's column blocking -----------------------------------------
+    refill()
+    g.chebyshev_filter(Psi, m, wl.a, wl.b, wl.a0, col_block=col_block)
+    F = api.colmajor_to_numpy(Psi[idx])
+    t0 = time.time()
+    O = H.chebyshev_filter(X, m, wl.a, wl.b, wl.a0)
+    t_or = time.time() - t0
+    ef = col_err(F, O)
+    print(f"[parity] cfg{cfg} filter m={m}, {len(cols)} sampled columns of {ns} (oracle {t_or:.1f} s): {ef:.3e}")
+    assert ef <= TOL_COL and ef <= TIGHT
+    assert math.isfinite(float(torch.linalg.vector_norm(Psi)))
+    assert g.get_info("kernel_launches") > 0
+    g.close()
+    del Psi
+    torch.cuda.empty_cache()
+    print(f"[parity] cfg{cfg} full-size sampled parity done in {time.time() - t_start:.0f} s")
+
+
+def test_config2_fullsize_sampled(torch, api):
+    fullsize_parity(torch, api, 2, n_random_cols=14, n_gram=12, n_random_rows=48, check_invariants=True)
+
+
+def test_config3_fullsize_sampled(torch, api):
+    fullsize_parity(torch, api, 3, n_random_cols=8, n_gram=10, n_random_rows=32, check_invariants=True)
+
+
+def test_config4_fullsize_sampled(torch, api):
+    free, total = torch.cuda.mem_get_info()
+    if total < 150e9:
+        pytest.skip("config 4 needs a 180 GB B200")
+    fullsize_parity(torch, api, 4, n_random_cols=8, n_gram=10, n_random_rows=32, check_invariants=False)
