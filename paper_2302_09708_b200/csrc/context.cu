@@ -94,6 +94,7 @@ void free_tables(sparc_gpu_ctx *c)
     cudaFree(c->d_supp_ptr); cudaFree(c->d_supp_idx); cudaFree(c->d_n_proj); cudaFree(c->d_proj_ofs);
     cudaFree(c->d_chi_ptr); cudaFree(c->d_chi); cudaFree(c->d_gamma); cudaFree(c->d_cov_idx);
     cudaFree(c->d_cov_ptr); cudaFree(c->d_cov_ent); cudaFree(c->d_veff);
+    nlb_free(c);
 }
 
 int validate_desc(const sparc_gpu_desc *d)
@@ -160,7 +161,7 @@ int ws_layout(const sparc_gpu_ctx *c, int op, int64_t ns, int64_t block, WsLayou
         L->off_w = off;
         if (op != SPARC_GPU_OP_HAMILTONIAN_APPLY) off += round_up_i64(L->ldw * cb * 8, A);
         L->off_d = off;
-        off += round_up_i64((int64_t)std::max(c->n_proj_total, 1) * cb * 8, A);
+        off += round_up_i64(2 * (int64_t)std::max(c->n_proj_total, 1) * nlb_c_cols(cb) * 8, A);
         L->off_g = off;
         if (op == SPARC_GPU_OP_PROJECT) {
             off += round_up_i64(std::max(gemm_tn_ws_bytes(c, ns, cb, c->nd), gemm_tn_ws_bytes(c, ns, ns, c->nd)), A);
@@ -183,9 +184,9 @@ int ws_layout(const sparc_gpu_ctx *c, int op, int64_t ns, int64_t block, WsLayou
     return SPARC_GPU_SUCCESS;
 }
 
-// Out = alpha (H X + shift X) + beta Prev on one column block: fused local pass + nonlocal pair.
-int h_pass(sparc_gpu_ctx *c, const double *X, int64_t ldx, double *Out, int64_t ldo, const double *Prev,
-           int64_t ldp, int64_t ncols, double alpha, double shift, double beta, double *D, cudaStream_t st)
+// Out = alpha (H_loc X + shift X) + beta Prev on one column block: the fused local pass (stencil + Veff + axpy).
+int local_pass(sparc_gpu_ctx *c, const double *X, int64_t ldx, double *Out, int64_t ldo, const double *Prev,
+               int64_t ldp, int64_t ncols, double alpha, double shift, double beta, cudaStream_t st)
 {
     int path = c->opt_stencil_path;
     if (path == 0) path = stencil_tma_supported(c, X, ldx, Out, ldo, Prev, ldp) ? 2 : 1;
@@ -195,14 +196,42 @@ int h_pass(sparc_gpu_ctx *c, const double *X, int64_t ldx, double *Out, int64_t 
         SPARC_TRY(launch_stencil_generic(c, X, ldx, Out, ldo, Prev, ldp, ncols, alpha, shift, beta, st));
     }
     c->stencil_path_last = path;
-    if (c->opt_nonlocal && c->n_atoms > 0 && c->n_proj_total > 0 && c->supp_total > 0) {
-        if (c->opt_nonlocal_mode == 1) {
-            SPARC_TRY(launch_nl_project(c, X, ldx, ncols, alpha, D, st));
-            SPARC_TRY(launch_nl_pull(c, D, Out, ldo, ncols, st));
-        } else {
-            SPARC_TRY(launch_nl_fused(c, X, ldx, Out, ldo, ncols, alpha, st));
-        }
+    return SPARC_GPU_SUCCESS;
+}
+
+// Nonlocal path of a pass that reads X and updates Out: -1 none, 1 project + pull, 2 per-atom fused, 3 brick.
+int effective_nl_mode(const sparc_gpu_ctx *c, const double *X, int64_t ldx, const double *Out, int64_t ldo)
+{
+    if (!c->opt_nonlocal || c->n_atoms <= 0 || c->n_proj_total <= 0 || c->supp_total <= 0) return -1;
+    if (c->opt_nonlocal_mode != 0) return c->opt_nonlocal_mode;
+    return (nlb_supported(c, X, ldx) && nlb_supported(c, Out, ldo)) ? 3 : 2;
+}
+
+// Out += alpha V_nl X with the per-atom kernels (modes 1, 2)
+int nl_pass_per_atom(sparc_gpu_ctx *c, int mode, const double *X, int64_t ldx, double *Out, int64_t ldo, int64_t ncols,
+                     double alpha, double *D, cudaStream_t st)
+{
+    if (mode == 1) {
+        SPARC_TRY(launch_nl_project(c, X, ldx, ncols, alpha, D, st));
+        SPARC_TRY(launch_nl_pull(c, D, Out, ldo, ncols, st));
+    } else {
+        SPARC_TRY(launch_nl_fused(c, X, ldx, Out, ldo, ncols, alpha, st));
     }
+    return SPARC_GPU_SUCCESS;
+}
+
+// Y = H X on one column block (D: workspace of 2 * n_proj_total * ncols doubles)
+int h_apply_block(sparc_gpu_ctx *c, const double *X, int64_t ldx, double *Y, int64_t ldy, int64_t ncols, double *D,
+                  cudaStream_t st)
+{
+    const int mode = effective_nl_mode(c, X, ldx, Y, ldy);
+    if (mode == 3) {      // chi^T X first (X may not be read after Y is written when they alias; they never do here)
+        SPARC_CUDA_TRY(cudaMemsetAsync(D, 0, (size_t)c->n_proj_total * nlb_c_cols(ncols) * 8, st));
+        SPARC_TRY(launch_nl_brick(c, 1, const_cast<double *>(X), ldx, ncols, 0.0, nullptr, D, st));
+    }
+    SPARC_TRY(local_pass(c, X, ldx, Y, ldy, nullptr, 0, ncols, 1.0, 0.0, 0.0, st));
+    if (mode == 3) SPARC_TRY(launch_nl_brick(c, 2, Y, ldy, ncols, 1.0, D, nullptr, st));
+    else if (mode > 0) SPARC_TRY(nl_pass_per_atom(c, mode, X, ldx, Y, ldy, ncols, 1.0, D, st));
     return SPARC_GPU_SUCCESS;
 }
 
@@ -328,6 +357,7 @@ int sparc_gpu_create(const sparc_gpu_desc *desc, sparc_gpu_ctx **out)
         if ((st = upload(&c->d_cov_idx, cov_idx.data(), cov_idx.size()))) break;
         if ((st = upload(&c->d_cov_ptr, cov_ptr.data(), cov_ptr.size()))) break;
         if ((st = upload(&c->d_cov_ent, ent.data(), ent.size()))) break;
+        if ((st = nlb_build(c, desc))) break;
     } while (0);
     if (st != SPARC_GPU_SUCCESS) { (void)cudaGetLastError(); free_tables(c); delete c->prof; delete c; return st; }
     *out = c;
@@ -360,7 +390,7 @@ int sparc_gpu_set_option(sparc_gpu_ctx *ctx, const char *key, int64_t value)
 {
     if (!ctx || !key) return SPARC_GPU_INVALID_ARG;
     if (!strcmp(key, "stencil_path")) { if (value < 0 || value > 2) return SPARC_GPU_INVALID_ARG; ctx->opt_stencil_path = (int)value; return 0; }
-    if (!strcmp(key, "nonlocal_mode")) { if (value < 0 || value > 1) return SPARC_GPU_INVALID_ARG; ctx->opt_nonlocal_mode = (int)value; return 0; }
+    if (!strcmp(key, "nonlocal_mode")) { if (value < 0 || value > 3) return SPARC_GPU_INVALID_ARG; ctx->opt_nonlocal_mode = (int)value; return 0; }
     if (!strcmp(key, "nonlocal")) { ctx->opt_nonlocal = value ? 1 : 0; return 0; }
     if (!strcmp(key, "profile")) { if (!ctx->prof) return SPARC_GPU_OUT_OF_MEMORY; ctx->prof->on = value != 0; return 0; }
     if (!strcmp(key, "profile_reset")) {
@@ -386,6 +416,9 @@ int sparc_gpu_get_info(const sparc_gpu_ctx *ctx, const char *key, int64_t *value
     if (!strcmp(key, "covered_points")) { *value = ctx->n_covered; return 0; }
     if (!strcmp(key, "stencil_path_last")) { *value = ctx->stencil_path_last; return 0; }
     if (!strcmp(key, "sm_count")) { *value = ctx->sm_count; return 0; }
+    if (!strcmp(key, "nl_brick")) { *value = ctx->nlb.ok; return 0; }
+    if (!strcmp(key, "nl_brick_blocks")) { *value = ctx->nlb.n_blocks; return 0; }
+    if (!strcmp(key, "nl_brick_active")) { *value = ctx->nlb.n_active; return 0; }
     if (!strncmp(key, "prof_ns:", 8) || !strncmp(key, "prof_count:", 11)) {
         if (!ctx->prof) return SPARC_GPU_OUT_OF_MEMORY;
         const bool is_ns = key[5] == 'n';
@@ -419,8 +452,7 @@ int sparc_gpu_hamiltonian_apply(sparc_gpu_ctx *ctx, const double *X, int64_t ldx
     double *D = (double *)((char *)ws + L.off_d);
     for (int64_t j0 = 0; j0 < ncols; j0 += L.block) {
         const int64_t nb = std::min(L.block, ncols - j0);
-        SPARC_TRY(h_pass(ctx, X + j0 * ldx, ldx, Y + j0 * ldy, ldy, nullptr, 0, nb, 1.0, 0.0, 0.0, D,
-                         (cudaStream_t)stream));
+        SPARC_TRY(h_apply_block(ctx, X + j0 * ldx, ldx, Y + j0 * ldy, ldy, nb, D, (cudaStream_t)stream));
     }
     return SPARC_GPU_SUCCESS;
 }
@@ -445,15 +477,29 @@ int sparc_gpu_chebyshev_filter(sparc_gpu_ctx *ctx, double *Psi, int64_t ld, int6
         double *bufA = Psi + j0 * ld;     // holds Y_{k-1} (k odd) / Y_k (k even)
         double *cur = bufA, *oth = W;
         int64_t ldc = ld, ldo = L.ldw;
-        // k = 1:  oth = (sigma1/e)(H cur - c cur)
-        SPARC_TRY(h_pass(ctx, cur, ldc, oth, ldo, nullptr, 0, nb, sigma1 / e, -c, 0.0, D, st));
+        // one degree step: oth <- alpha (H cur - c cur) + beta oth.  With the brick kernel the nonlocal term of step k
+        // and the projection chi^T Psi_k needed by step k + 1 share one read-modify-write of oth.
+        const int mode = effective_nl_mode(ctx, cur, ldc, oth, ldo);
+        const size_t cbytes = (size_t)ctx->n_proj_total * nlb_c_cols(nb) * 8;
+        double *Cb[2] = {D, D + (int64_t)ctx->n_proj_total * nlb_c_cols(nb)};
+        if (mode == 3) {
+            SPARC_CUDA_TRY(cudaMemsetAsync(Cb[0], 0, cbytes, st));
+            SPARC_TRY(launch_nl_brick(ctx, 1, cur, ldc, nb, 0.0, nullptr, Cb[0], st));
+        }
         double sigma = sigma1;
-        std::swap(cur, oth); std::swap(ldc, ldo);
-        for (int k = 2; k <= degree; ++k) {
+        for (int k = 1; k <= degree; ++k) {
             const double sigma2 = 1.0 / (tau - sigma);
-            // oth (= Y_{k-2}) <- (2 sigma2/e)(H cur - c cur) - sigma sigma2 * oth
-            SPARC_TRY(h_pass(ctx, cur, ldc, oth, ldo, oth, ldo, nb, 2.0 * sigma2 / e, -c, -(sigma * sigma2), D, st));
-            sigma = sigma2;
+            const double alpha = (k == 1) ? sigma1 / e : 2.0 * sigma2 / e;
+            const double beta = (k == 1) ? 0.0 : -(sigma * sigma2);
+            SPARC_TRY(local_pass(ctx, cur, ldc, oth, ldo, k == 1 ? nullptr : oth, ldo, nb, alpha, -c, beta, st));
+            if (mode == 3) {
+                const bool last = (k == degree);
+                if (!last) SPARC_CUDA_TRY(cudaMemsetAsync(Cb[k & 1], 0, cbytes, st));
+                SPARC_TRY(launch_nl_brick(ctx, last ? 2 : 3, oth, ldo, nb, alpha, Cb[(k - 1) & 1], Cb[k & 1], st));
+            } else if (mode > 0) {
+                SPARC_TRY(nl_pass_per_atom(ctx, mode, cur, ldc, oth, ldo, nb, alpha, D, st));
+            }
+            if (k > 1) sigma = sigma2;
             std::swap(cur, oth); std::swap(ldc, ldo);
         }
         if (cur != bufA) SPARC_TRY(launch_copy_2d(ctx, bufA, ld, cur, ldc, ctx->nd, nb, st));
@@ -476,7 +522,7 @@ int sparc_gpu_project(sparc_gpu_ctx *ctx, const double *Psi, int64_t ld, int64_t
     void *G = (char *)ws + L.off_g;
     for (int64_t j0 = 0; j0 < ns; j0 += L.block) {
         const int64_t nb = std::min(L.block, ns - j0);
-        SPARC_TRY(h_pass(ctx, Psi + j0 * ld, ld, Y, L.ldw, nullptr, 0, nb, 1.0, 0.0, 0.0, D, st));
+        SPARC_TRY(h_apply_block(ctx, Psi + j0 * ld, ld, Y, L.ldw, nb, D, st));
         // Hs[:, j0:j0+nb] = Psi^T Y_block
         SPARC_TRY(launch_gemm_tn(ctx, Psi, ld, Y, L.ldw, Hs + j0 * ns, ns, ns, nb, ctx->nd, G, st));
     }

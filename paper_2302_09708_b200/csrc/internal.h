@@ -25,6 +25,20 @@ struct CoverEntry {
     int32_t pofs_p;    // (offset of atom J's first projector in D) << 8 | P_J
 };
 
+// Tables of the brick-tiled nonlocal kernel (nonlocal_brick.cu): built at create, immutable.
+struct NlBrick {
+    int ok = 0;                // 0: grid does not meet the preconditions, per-atom kernels are used
+    int pclass = 0;            // 4 or 9: projector-count class the blocks are laid out for
+    int bx = 0, by = 0, bz = 0;   // brick shape, bx * by * bz = 256
+    int32_t n_active = 0;      // bricks met by at least one support
+    int64_t n_blocks = 0;      // chi blocks = touched (brick, atom, octet) triples
+    int32_t *d_org = nullptr;      // [n_active][4]: x0, y0, z0, union octet mask
+    int32_t *d_job_ptr = nullptr;  // [n_active + 1]
+    void *d_jobs = nullptr;        // BrickJob[]
+    double *d_pull = nullptr;      // pull-fragment blocks
+    double *d_proj = nullptr;      // projection-fragment blocks
+};
+
 struct sparc_gpu_ctx {
     int device;
     int sm_count;
@@ -52,13 +66,15 @@ struct sparc_gpu_ctx {
     int32_t *d_cov_idx;        // [n_covered] grid index of each covered point (ascending)
     int64_t *d_cov_ptr;        // [n_covered+1] offsets into d_cov_ent
     CoverEntry *d_cov_ent;     // [supp_total]
+    NlBrick nlb;
     // local potential
     double *d_veff;            // [nd]
     // options
     int opt_stencil_path;      // 0 auto, 1 generic, 2 TMA
     int opt_nonlocal;          // 1 on
     int opt_gemm_path;         // 0 auto, 1 simple, 2 DMMA
-    int opt_nonlocal_mode;     // 0 fused per-atom kernel with atomic scatter, 1 project + pull (deterministic)
+    int opt_nonlocal_mode;     // 0 auto (brick kernel when supported, else 2), 1 project + pull (deterministic),
+                               // 2 fused per-atom kernel with atomic scatter, 3 brick kernel or UNSUPPORTED
     int opt_stencil_ay;        // 0 auto, 1 or 2: rows per consumer thread of the TMA stencil kernel
     int opt_stencil_ty;        // 0 auto, else forced tile rows of the TMA stencil kernel
     int opt_stencil_stages;    // 0 auto, else cap on the smem ring depth
@@ -75,7 +91,7 @@ struct sparc_gpu_ctx {
 // Kernel kinds for the event profiler and the launch counters.
 enum KernelKind {
     KK_STENCIL_GENERIC = 0, KK_STENCIL_TMA = 1, KK_NL_PROJECT = 2, KK_NL_PULL = 3, KK_GEMM_TN = 4,
-    KK_GEMM_NN = 5, KK_SPLITK_REDUCE = 6, KK_COPY2D = 7, KK_NL_FUSED = 8, KK_COUNT = 9
+    KK_GEMM_NN = 5, KK_SPLITK_REDUCE = 6, KK_COPY2D = 7, KK_NL_FUSED = 8, KK_NL_BRICK = 9, KK_COUNT = 10
 };
 // Bracket one kernel launch with events when profiling is on (no-ops otherwise); both bump the counters.
 void prof_begin(sparc_gpu_ctx *ctx, int kind, cudaStream_t st);
@@ -122,6 +138,18 @@ int launch_nl_pull(sparc_gpu_ctx *ctx, const double *D, double *Out, int64_t ldo
 // scatter (default nonlocal path; not bitwise reproducible across runs, see option "nonlocal_mode")
 int launch_nl_fused(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double *Out, int64_t ldo, int64_t ncols,
                     double scale, cudaStream_t st);
+
+// Brick-tiled nonlocal kernel (nonlocal_brick.cu).  C buffers hold the raw sums chi_J^T Psi atom-major, element
+// (J, q, col) at po_J * nlb_c_cols(ncols) + col * P_J + q: n_proj_total * nlb_c_cols(ncols) doubles each.
+static inline int64_t nlb_c_cols(int64_t ncols) { return (ncols + 63) / 64 * 64; }
+//   mode 1 (project): c_out += chi^T X                  (X read only; c_out zeroed by the caller)
+//   mode 2 (pull)   : Out += chi (scale Gamma c_in)
+//   mode 3 (both)   : Out += chi (scale Gamma c_in), then c_out += chi^T Out
+int nlb_build(sparc_gpu_ctx *ctx, const sparc_gpu_desc *d);
+void nlb_free(sparc_gpu_ctx *ctx);
+bool nlb_supported(const sparc_gpu_ctx *ctx, const double *X, int64_t ld);
+int launch_nl_brick(sparc_gpu_ctx *ctx, int mode, double *XorOut, int64_t ld, int64_t ncols, double scale,
+                    const double *c_in, double *c_out, cudaStream_t st);
 
 // C (M x N, col-major, ldc) = A^T B, A: K x M (lda), B: K x N (ldb), contraction over K rows.
 // ws: split-K partials (gemm_tn_ws_bytes).  symmetric_out: A == B, fill lower from upper.

@@ -1,0 +1,512 @@
+// nonlocal_brick.cu -- brick-tiled Kleinman-Bylander nonlocal term on the FP64 tensor pipe (default nonlocal path).
+//
+//   V_nl X = sum_J S_J^T chi_J diag(gamma_J) chi_J^T S_J X
+//
+// The per-atom formulation gathers X at each atom's support and scatter-adds with atomics: 8c + 16c bytes and one
+// atomic per (support row, column) (c = coverage, 4-5 at configs 3-4).  Here the grid is cut into bricks of 256
+// points (BX x BY x BZ, x fastest) and one CTA owns (brick, 64 columns): it reads the 256 x 64 tile of Out once into
+// tensor-core accumulator fragments, adds the contribution of EVERY atom whose support meets the brick
+// ("pull": Out^T[col, pt] += D_J^T[col, q] chi_J^T[q, pt], DMMA m8n8k4), writes the tile back once, and -- the tile
+// now being the final Psi_{k+1} -- contracts it with the same chi blocks for the NEXT degree step
+// ("project": C_J[q, col] += chi_J^T[q, pt] Out[pt, col]), so that the nonlocal term costs one 16 B read-modify-write
+// of Out per degree step and one atomic per (brick, atom, projector, column).  The accumulator fragment of the pull
+// is, register for register, the B operand of the projection (k index = point pair), so no layout change is needed.
+//
+// Tables built at create (host): for every (brick, atom) pair a 32-bit mask of the brick's 8-point octets the atom
+// touches, and per touched octet a dense block of chi values already permuted into DMMA fragment order (zeros where
+// the atom does not cover a point; gamma folded into the pull blocks).  Blocks of one (brick, atom) pair are
+// contiguous; a producer warp streams them (and the 64-column slice of C_J) into a shared-memory byte ring with
+// cp.async.bulk, up to 16 (brick, atom) jobs ahead of the eight consumer warps (full / empty mbarriers).
+//
+// The 9th projector of an s+p+d atom is applied as a rank-1 FMA update beside the two k-steps of DMMA (a third
+// k-step would be 3/4 padding).
+#include <algorithm>
+#include <cstdio>
+#include <unordered_map>
+#include <vector>
+
+#include "internal.h"
+
+namespace {
+
+constexpr int NB_PTS = 256;        // points per brick
+constexpr int NB_OCT = 32;         // octets per brick (bit mask width)
+constexpr int NLB_WARPS = 16;      // consumer warps: 8 column slices x 2 brick halves
+constexpr int NB_HOCT = 16;        // octets per brick half (one consumer warp's share)
+constexpr int NLB_COLS = 64;       // columns per CTA: 8 per warp
+
+struct BrickJob {                  // one (brick, atom) pair
+    int32_t atom;
+    uint32_t mask;                 // octets of the brick this atom touches
+    int64_t blk0;                  // index of its first chi block
+    int32_t po;                    // offset of the atom's first projector (prefix sum of P_J)
+    int32_t pj;                    // P_J
+};
+
+struct BrickParams {
+    const int32_t *brick_org;      // [n_active][3] origin (x0, y0, z0)
+    const int32_t *job_ptr;        // [n_active + 1]
+    const BrickJob *jobs;
+    const double *blk_pull;        // [n_blocks][PULL_SZ]
+    const double *blk_proj;        // [n_blocks][PROJ_SZ]
+    const double *src;             // X (project-only) or Out (pull): N_d x ncols, ld
+    double *dst;                   // Out (pull variants)
+    int64_t ld;
+    // C buffers hold the raw sums chi_J^T Psi atom-major: element (J, q, col) at po_J * ncp + col * P_J + q
+    const double *c_in;            // chi^T Psi_k of the previous pass (pull)
+    double *c_out;                 // accumulated chi^T Psi_{k+1} (project), zeroed by the caller
+    int64_t ncp;                   // padded column count of the C buffers (multiple of 64)
+    int32_t ncols;
+    int32_t ncolgroups;
+    int32_t nx, ny, nz;
+    int32_t bx, by, bz;
+    double scale;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" ::"r"(smem_u32(bar)),
+                 "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "NLB_WAIT:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra NLB_DONE;\n\t"
+        "bra NLB_WAIT;\n\t"
+        "NLB_DONE:\n\t"
+        "}" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
+
+
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(smem_u32(bar)) : "memory");
+}
+
+constexpr int NLB_SLOTS = 16;                 // jobs in flight (mbarrier pairs)
+constexpr int NLB_RING_BYTES = 160 * 1024;    // byte ring the producer warp streams chi blocks (+ C slices) through
+
+// KP: DMMA k-steps of the pull (projectors 0 .. 4 KP - 1); MT: 8-projector m-tiles of the projection; R1: projector
+// number 8 applied as a rank-1 FMA update (s+p+d atoms: P = 9).  DO_PULL / DO_PROJ select the three variants:
+// project only (C_0 of a filter call, first half of H X), pull only (last degree step, second half of H X), both.
+// Warps 0-15 are consumers (8 columns x one half of the brick each), warp 16 is the producer: it walks the brick's job list ahead of the
+// consumers and streams, per (brick, atom) job, the chi blocks (and for a pull job the 64-column slice of C_J) into a
+// byte ring with cp.async.bulk; full/empty mbarriers per slot.
+template <int KP, int MT, bool R1, bool DO_PULL, bool DO_PROJ>
+__global__ void __launch_bounds__((NLB_WARPS + 1) * 32, 1)
+nl_brick_kernel(const BrickParams p)
+{
+    constexpr int PULL_SZ = KP * 32 + (R1 ? 8 : 0);
+    constexpr int PROJ_SZ = MT * 64 + (R1 ? 8 : 0);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    unsigned char *ring = smem_raw;                                                   // [NLB_RING_BYTES]
+    int32_t *pt_off = reinterpret_cast<int32_t *>(ring + NLB_RING_BYTES);             // [NB_PTS] grid index, -1 outside
+    uint64_t *full = reinterpret_cast<uint64_t *>(pt_off + NB_PTS);                   // [NLB_SLOTS]
+    uint64_t *empty = full + NLB_SLOTS;                                               // [NLB_SLOTS]
+    int32_t *slot_off = reinterpret_cast<int32_t *>(empty + NLB_SLOTS);               // [NLB_SLOTS] ring offset of the job
+    uint32_t *slot_mask = reinterpret_cast<uint32_t *>(slot_off + NLB_SLOTS);         // [NLB_SLOTS]
+    int32_t *slot_pj = reinterpret_cast<int32_t *>(slot_mask + NLB_SLOTS);            // [NLB_SLOTS] P_J
+    int32_t *slot_po = slot_pj + NLB_SLOTS;                                           // [NLB_SLOTS] projector offset of J
+    int32_t *slot_size = slot_po + NLB_SLOTS;                                         // [NLB_SLOTS] ring bytes (producer only)
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int lq = lane & 3, lr = lane >> 2;
+    const int brick = blockIdx.x / p.ncolgroups;
+    const int cg = blockIdx.x - brick * p.ncolgroups;
+    const int x0 = p.brick_org[4 * brick], y0 = p.brick_org[4 * brick + 1], z0 = p.brick_org[4 * brick + 2];
+    const uint32_t umask = (uint32_t)p.brick_org[4 * brick + 3];
+    if (tid < NB_PTS) {
+        const int lx = tid % p.bx, ly = (tid / p.bx) % p.by, lz = tid / (p.bx * p.by);
+        const int x = x0 + lx, y = y0 + ly, z = z0 + lz;
+        pt_off[tid] = (y < p.ny && z < p.nz) ? x + p.nx * (y + p.ny * z) : -1;
+    }
+    if (tid == 0) {
+        for (int s = 0; s < NLB_SLOTS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NLB_WARPS); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    const int j0 = p.job_ptr[brick];
+    const int na = p.job_ptr[brick + 1] - j0;
+    const int njobs = (DO_PULL ? na : 0) + (DO_PROJ ? na : 0);
+
+    if (warp == NLB_WARPS) {
+        // ================================ producer warp ==========================================================
+        // lanes fetch 32 job descriptors at a time; lane 0 allocates ring space in order and issues the copies
+        int head = 0, used = 0, freed = 0;
+        for (int jb = 0; jb < njobs; jb += 32) {
+            const int jmine = jb + lane;
+            BrickJob job = {0, 0u, 0, 0, 0};
+            if (jmine < njobs) job = p.jobs[j0 + (jmine < na ? jmine : jmine - na)];
+            const int cnt = min(32, njobs - jb);
+            for (int i = 0; i < cnt; ++i) {
+                const int jj = jb + i;
+                const uint32_t mask = __shfl_sync(0xffffffffu, job.mask, i);
+                const int pj = __shfl_sync(0xffffffffu, job.pj, i);
+                const int po = __shfl_sync(0xffffffffu, job.po, i);
+                const long long blk0 = __shfl_sync(0xffffffffu, (long long)job.blk0, i);
+                if (lane != 0) continue;
+                const bool pull = DO_PULL && jj < na;
+                const uint32_t blk_bytes = (uint32_t)__popc(mask) * (uint32_t)(pull ? PULL_SZ : PROJ_SZ) * 8u;
+                const uint32_t c_bytes = pull ? (uint32_t)(NLB_COLS * pj * 8) : 0u;
+                int need = (int)((blk_bytes + c_bytes + 127u) & ~127u);
+                const bool wrap = head + need > NLB_RING_BYTES;                       // no job straddles the ring end
+                const int skip = wrap ? NLB_RING_BYTES - head : 0;
+                while (jj - freed >= NLB_SLOTS || used + need + skip > NLB_RING_BYTES) {
+                    const int fs = freed % NLB_SLOTS;
+                    mbar_wait(&empty[fs], (uint32_t)((freed / NLB_SLOTS) & 1));
+                    used -= slot_size[fs];
+                    ++freed;
+                }
+                if (wrap) head = 0;
+                const int slot = jj % NLB_SLOTS;
+#ifdef NLB_DEBUG
+                if (na >= 17 && cg == 0 && jj >= 13) printf("P b=%d jj=%d slot=%d head=%d need=%d skip=%d used=%d freed=%d mask=%08x pj=%d po=%d blk0=%lld bytes=%u+%u\n", brick, jj, slot, head, need, skip, used, freed, mask, pj, po, blk0, blk_bytes, c_bytes);
+#endif
+                slot_size[slot] = need + skip;
+                used += need + skip;
+                slot_off[slot] = head; slot_mask[slot] = mask; slot_pj[slot] = pj; slot_po[slot] = po;
+                mbar_expect_tx(&full[slot], blk_bytes + c_bytes);
+                const double *src = pull ? p.blk_pull + blk0 * PULL_SZ : p.blk_proj + blk0 * PROJ_SZ;
+                bulk_g2s(ring + head, src, blk_bytes, &full[slot]);
+                if (pull)
+                    bulk_g2s(ring + head + blk_bytes, p.c_in + (int64_t)po * p.ncp + (int64_t)cg * NLB_COLS * pj, c_bytes,
+                             &full[slot]);
+                head += need;
+            }
+        }
+        return;
+    }
+
+    // ==================================== consumer warps ============================================================
+    // the 128 x 8 tile of this warp (octets 16 half .. 16 half + 15), in accumulator-fragment order: lane (lr, lq)
+    // holds column colw + lr, points 2 lq and 2 lq + 1 of every octet
+    const int half = warp >> 3;
+    const int colw = cg * NLB_COLS + (warp & 7) * 8;
+    const int col = colw + lr;
+    const bool colv = col < p.ncols;
+    const uint32_t umask_h = (umask >> (16 * half)) & 0xffffu;
+    const int32_t *pt_h = pt_off + 128 * half + 2 * lq;
+    const double *srcc = p.src + (int64_t)(colv ? col : 0) * p.ld;
+    double2 c[NB_HOCT];
+#pragma unroll
+    for (int o = 0; o < NB_HOCT; ++o) {
+        c[o] = make_double2(0.0, 0.0);
+        if (umask_h & (1u << o)) {
+            const int off = pt_h[8 * o];
+            if (off >= 0 && colv) c[o] = *reinterpret_cast<const double2 *>(srcc + off);
+        }
+    }
+
+    for (int jj = 0; jj < njobs; ++jj) {
+        const int slot = jj % NLB_SLOTS;
+        const bool pull = DO_PULL && jj < na;
+        mbar_wait(&full[slot], (uint32_t)((jj / NLB_SLOTS) & 1));
+        const uint32_t mask_all = slot_mask[slot];
+        const uint32_t mask = (mask_all >> (16 * half)) & 0xffffu;
+        const int blk_h = half ? __popc(mask_all & 0xffffu) : 0;          // first block of this half
+        const int PJ = slot_pj[slot], po = slot_po[slot];
+        const double *base = reinterpret_cast<const double *>(ring + slot_off[slot]);
+#ifdef NLB_DEBUG
+        if (na >= 17 && cg == 0 && jj >= 13 && lane == 0 && (warp == 0 || warp == 15)) printf("C b=%d w=%d jj=%d slot=%d off=%d mask=%08x pj=%d po=%d\n", brick, warp, jj, slot, slot_off[slot], mask_all, PJ, po);
+#endif
+
+        if (pull) {
+            // A operand: D_J^T[col, q] = scale (chi_J^T Psi_k)[q, col]   (gamma_q is folded into the pull blocks)
+            const double *cs = base + __popc(mask_all) * PULL_SZ + ((warp & 7) * 8 + lr) * PJ;
+            double dA[KP], d8 = 0.0;
+#pragma unroll
+            for (int ks = 0; ks < KP; ++ks) {
+                const int q = 4 * ks + lq;
+                dA[ks] = (q < PJ && (!R1 || q < 8)) ? p.scale * cs[q] : 0.0;
+            }
+            if (R1) d8 = (8 < PJ) ? p.scale * cs[8] : 0.0;
+            int blk = blk_h;
+#pragma unroll
+            for (int o = 0; o < NB_HOCT; ++o) {
+                if (mask & (1u << o)) {
+                    const double *b = base + blk * PULL_SZ;
+#pragma unroll
+                    for (int ks = 0; ks < KP; ++ks) dmma884(c[o].x, c[o].y, dA[ks], b[ks * 32 + lane]);
+                    if (R1) {
+                        const double2 x8 = *reinterpret_cast<const double2 *>(b + KP * 32 + 2 * lq);
+                        c[o].x = fma(d8, x8.x, c[o].x);
+                        c[o].y = fma(d8, x8.y, c[o].y);
+                    }
+                    ++blk;
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[slot]);
+            if (jj == na - 1) {                            // all atoms pulled: the tile is the final Out
+                double *dstc = p.dst + (int64_t)(colv ? col : 0) * p.ld;
+#pragma unroll
+                for (int o = 0; o < NB_HOCT; ++o) {
+                    if (umask_h & (1u << o)) {
+                        const int off = pt_h[8 * o];
+                        if (off >= 0 && colv) *reinterpret_cast<double2 *>(dstc + off) = c[o];
+                    }
+                }
+            }
+        } else {
+            // C_J[q, col] += sum_pt chi_J[pt, q] Out[pt, col]; two independent accumulator sets shorten the DMMA chains
+            double acc[2][MT][2], p8[2];
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                p8[s] = 0.0;
+#pragma unroll
+                for (int mt = 0; mt < MT; ++mt) acc[s][mt][0] = acc[s][mt][1] = 0.0;
+            }
+            int blk = blk_h;
+#pragma unroll
+            for (int o = 0; o < NB_HOCT; ++o) {
+                if (mask & (1u << o)) {
+                    const double *b = base + blk * PROJ_SZ;
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt) {
+                        dmma884(acc[o & 1][mt][0], acc[o & 1][mt][1], b[(2 * mt) * 32 + lane], c[o].x);
+                        dmma884(acc[o & 1][mt][0], acc[o & 1][mt][1], b[(2 * mt + 1) * 32 + lane], c[o].y);
+                    }
+                    if (R1) {
+                        const double2 x8 = *reinterpret_cast<const double2 *>(b + MT * 64 + 2 * lq);
+                        p8[o & 1] = fma(x8.x, c[o].x, p8[o & 1]);
+                        p8[o & 1] = fma(x8.y, c[o].y, p8[o & 1]);
+                    }
+                    ++blk;
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[slot]);
+            double *cout = p.c_out + (int64_t)po * p.ncp;
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) {
+                const double v0 = acc[0][mt][0] + acc[1][mt][0];
+                const double v1 = acc[0][mt][1] + acc[1][mt][1];
+                const int q = mt * 8 + lr;
+                const int ca = colw + 2 * lq;
+                if (q < PJ && (!R1 || q < 8)) {
+                    if (ca < p.ncols) atomicAdd(cout + (int64_t)ca * PJ + q, v0);
+                    if (ca + 1 < p.ncols) atomicAdd(cout + (int64_t)(ca + 1) * PJ + q, v1);
+                }
+            }
+            if (R1) {
+                double v = p8[0] + p8[1];
+                v += __shfl_xor_sync(0xffffffffu, v, 1);
+                v += __shfl_xor_sync(0xffffffffu, v, 2);
+                if (lq == 0 && colv && 8 < PJ) atomicAdd(cout + (int64_t)col * PJ + 8, v);
+            }
+        }
+    }
+}
+
+struct ClassInfo { int kp, mt, r1, pull_sz, proj_sz; };
+
+ClassInfo class_info(int pclass)
+{
+    if (pclass == 4) return {1, 1, 0, 32, 64};
+    return {2, 1, 1, 72, 72};
+}
+
+template <typename T>
+int upload_vec(T **dst, const std::vector<T> &v)
+{
+    *dst = nullptr;
+    if (v.empty()) return SPARC_GPU_SUCCESS;
+    SPARC_CUDA_TRY(cudaMalloc((void **)dst, v.size() * sizeof(T)));
+    SPARC_CUDA_TRY(cudaMemcpy(*dst, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return SPARC_GPU_SUCCESS;
+}
+
+}  // namespace
+
+// Build the brick tables from the descriptor (host pointers, already validated).  Leaves ctx->nlb.ok = 0 when the
+// grid does not meet the preconditions (even nx with a brick width dividing it); the per-atom kernels then serve.
+int nlb_build(sparc_gpu_ctx *ctx, const sparc_gpu_desc *d)
+{
+    NlBrick &B = ctx->nlb;
+    B.ok = 0;
+    const int nx = ctx->n[0], ny = ctx->n[1], nz = ctx->n[2];
+    if (ctx->n_atoms == 0 || ctx->n_proj_total == 0 || ctx->supp_total == 0) return SPARC_GPU_SUCCESS;
+    if (ctx->max_proj > 9) return SPARC_GPU_SUCCESS;      // l <= 2 (s+p+d); larger sets use the per-atom kernels
+    if (nx % 16 == 0) { B.bx = 16; B.by = 4; B.bz = 4; }
+    else if (nx % 8 == 0) { B.bx = 8; B.by = 8; B.bz = 4; }
+    else if (nx % 4 == 0) { B.bx = 4; B.by = 8; B.bz = 8; }
+    else if (nx % 2 == 0) { B.bx = 2; B.by = 16; B.bz = 8; }
+    else return SPARC_GPU_SUCCESS;
+    B.pclass = ctx->max_proj <= 4 ? 4 : 9;
+    const ClassInfo ci = class_info(B.pclass);
+    const int nbx = nx / B.bx, nby = (ny + B.by - 1) / B.by, nbz = (nz + B.bz - 1) / B.bz;
+    const int64_t nbricks = (int64_t)nbx * nby * nbz;
+    if (nbricks >= (int64_t)INT32_MAX) return SPARC_GPU_SUCCESS;
+
+    struct Pair { int32_t brick, atom; uint32_t mask; };
+    std::vector<Pair> pairs;
+    auto locate = [&](int32_t i, int32_t *brick, int *li) {
+        const int x = i % nx, y = (i / nx) % ny, z = i / (nx * ny);
+        const int bx = x / B.bx, by = y / B.by, bz = z / B.bz;
+        *brick = bx + nbx * (by + nby * bz);
+        *li = (x - bx * B.bx) + B.bx * ((y - by * B.by) + B.by * (z - bz * B.bz));
+    };
+    // pass 1: octet masks per (brick, atom)
+    for (int J = 0; J < ctx->n_atoms; ++J) {
+        if (d->n_proj[J] <= 0) continue;
+        std::unordered_map<int32_t, uint32_t> m;
+        for (int64_t t = d->supp_ptr[J]; t < d->supp_ptr[J + 1]; ++t) {
+            int32_t brick; int li;
+            locate(d->supp_idx[t], &brick, &li);
+            m[brick] |= 1u << (li >> 3);
+        }
+        for (auto &kv : m) pairs.push_back({kv.first, J, kv.second});
+    }
+    if (pairs.empty()) return SPARC_GPU_SUCCESS;
+    std::sort(pairs.begin(), pairs.end(), [](const Pair &a, const Pair &b) {
+        return a.brick != b.brick ? a.brick < b.brick : a.atom < b.atom;
+    });
+    std::vector<int32_t> pofs((size_t)ctx->n_atoms + 1, 0);
+    for (int J = 0; J < ctx->n_atoms; ++J) pofs[(size_t)J + 1] = pofs[(size_t)J] + d->n_proj[J];
+    std::vector<int32_t> org, job_ptr;
+    std::vector<BrickJob> jobs(pairs.size());
+    int64_t nblocks = 0;
+    for (size_t k = 0; k < pairs.size(); ++k) {
+        if (k == 0 || pairs[k].brick != pairs[k - 1].brick) {
+            const int32_t b = pairs[k].brick;
+            const int bx = b % nbx, by = (b / nbx) % nby, bz = b / (nbx * nby);
+            org.push_back(bx * B.bx); org.push_back(by * B.by); org.push_back(bz * B.bz); org.push_back(0);
+            job_ptr.push_back((int32_t)k);
+        }
+        org[org.size() - 1] |= (int32_t)pairs[k].mask;
+        jobs[k] = {pairs[k].atom, pairs[k].mask, nblocks, pofs[(size_t)pairs[k].atom], d->n_proj[pairs[k].atom]};
+        nblocks += __builtin_popcount(pairs[k].mask);
+    }
+    job_ptr.push_back((int32_t)pairs.size());
+    B.n_active = (int32_t)(job_ptr.size() - 1);
+    B.n_blocks = nblocks;
+
+    // pass 2: chi blocks in fragment order
+    std::vector<double> pull((size_t)nblocks * ci.pull_sz, 0.0), proj((size_t)nblocks * ci.proj_sz, 0.0);
+    // per atom: brick -> job index
+    std::vector<std::unordered_map<int32_t, int64_t>> jobof((size_t)ctx->n_atoms);
+    for (size_t k = 0; k < pairs.size(); ++k) jobof[(size_t)pairs[k].atom][pairs[k].brick] = (int64_t)k;
+    for (int J = 0; J < ctx->n_atoms; ++J) {
+        const int P = d->n_proj[J];
+        if (P <= 0) continue;
+        const int64_t s0 = d->supp_ptr[J], nJ = d->supp_ptr[J + 1] - s0;
+        const double *chi = d->chi + d->chi_ptr[J];
+        for (int64_t t = 0; t < nJ; ++t) {
+            int32_t brick; int li;
+            locate(d->supp_idx[s0 + t], &brick, &li);
+            const BrickJob &job = jobs[(size_t)jobof[(size_t)J][brick]];
+            const int o = li >> 3, r = li & 7;
+            const int64_t blk = job.blk0 + __builtin_popcount(job.mask & ((1u << o) - 1u));
+            double *bp = pull.data() + blk * ci.pull_sz;
+            double *bj = proj.data() + blk * ci.proj_sz;
+            for (int q = 0; q < P; ++q) {
+                const double v = chi[t + (int64_t)q * nJ];
+                const double vg = v * d->gamma[pofs[(size_t)J] + q];       // pull blocks carry chi * gamma
+                if (ci.r1 && q == 8) {
+                    bp[ci.kp * 32 + r] = vg;
+                    bj[ci.mt * 64 + r] = v;
+                    continue;
+                }
+                // pull B fragment of k-step q/4: lane = 4 * point + q % 4
+                bp[(q >> 2) * 32 + r * 4 + (q & 3)] = vg;
+                // projection A fragment (m-tile q/8, k-step r%2): lane = 4 * (q % 8) + r / 2
+                bj[(2 * (q >> 3) + (r & 1)) * 32 + (q & 7) * 4 + (r >> 1)] = v;
+            }
+        }
+    }
+    int st;
+    if ((st = upload_vec(&B.d_org, org))) return st;
+    if ((st = upload_vec(&B.d_job_ptr, job_ptr))) return st;
+    {
+        B.d_jobs = nullptr;
+        SPARC_CUDA_TRY(cudaMalloc(&B.d_jobs, jobs.size() * sizeof(BrickJob)));
+        SPARC_CUDA_TRY(cudaMemcpy(B.d_jobs, jobs.data(), jobs.size() * sizeof(BrickJob), cudaMemcpyHostToDevice));
+    }
+    if ((st = upload_vec(&B.d_pull, pull))) return st;
+    if ((st = upload_vec(&B.d_proj, proj))) return st;
+    B.ok = 1;
+    return SPARC_GPU_SUCCESS;
+}
+
+void nlb_free(sparc_gpu_ctx *ctx)
+{
+    NlBrick &B = ctx->nlb;
+    cudaFree(B.d_org); cudaFree(B.d_job_ptr); cudaFree(B.d_jobs); cudaFree(B.d_pull); cudaFree(B.d_proj);
+    B = NlBrick();
+}
+
+bool nlb_supported(const sparc_gpu_ctx *ctx, const double *X, int64_t ld)
+{
+    return ctx->nlb.ok && (((uintptr_t)X & 15) == 0) && (ld % 2 == 0);
+}
+
+namespace {
+
+template <int KP, int MT, bool R1>
+int launch_class(sparc_gpu_ctx *ctx, int mode, const BrickParams &P, unsigned grid, cudaStream_t st)
+{
+    constexpr size_t SMEM = (size_t)NLB_RING_BYTES + NB_PTS * 4 + NLB_SLOTS * (8 + 8 + 5 * 4);
+    void (*kern)(const BrickParams) = mode == 1 ? nl_brick_kernel<KP, MT, R1, false, true>
+                                      : mode == 2 ? nl_brick_kernel<KP, MT, R1, true, false>
+                                                  : nl_brick_kernel<KP, MT, R1, true, true>;
+    SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
+    prof_begin(ctx, KK_NL_BRICK, st);
+    kern<<<grid, (NLB_WARPS + 1) * 32, SMEM, st>>>(P);
+    prof_end(ctx, KK_NL_BRICK, st);
+    SPARC_CUDA_TRY(cudaGetLastError());
+    return SPARC_GPU_SUCCESS;
+}
+
+}  // namespace
+
+int launch_nl_brick(sparc_gpu_ctx *ctx, int mode, double *XorOut, int64_t ld, int64_t ncols, double scale,
+                    const double *c_in, double *c_out, cudaStream_t st)
+{
+    const NlBrick &B = ctx->nlb;
+    if (!nlb_supported(ctx, XorOut, ld) || mode < 1 || mode > 3) return SPARC_GPU_UNSUPPORTED;
+    if (ncols <= 0 || B.n_active == 0) return SPARC_GPU_SUCCESS;
+    const int64_t ngroups = (ncols + NLB_COLS - 1) / NLB_COLS;
+    if ((int64_t)B.n_active * ngroups >= (int64_t)INT32_MAX) return SPARC_GPU_UNSUPPORTED;
+    BrickParams P;
+    P.brick_org = B.d_org; P.job_ptr = B.d_job_ptr; P.jobs = (const BrickJob *)B.d_jobs;
+    P.blk_pull = B.d_pull; P.blk_proj = B.d_proj;
+    P.src = XorOut; P.dst = XorOut; P.ld = ld;
+    P.c_in = c_in; P.c_out = c_out;
+    P.ncp = nlb_c_cols(ncols);
+    P.ncols = (int32_t)ncols;
+    P.ncolgroups = (int32_t)ngroups;
+    P.nx = ctx->n[0]; P.ny = ctx->n[1]; P.nz = ctx->n[2];
+    P.bx = B.bx; P.by = B.by; P.bz = B.bz;
+    P.scale = scale;
+    const unsigned grid = (unsigned)((int64_t)B.n_active * ngroups);
+    if (B.pclass == 4) SPARC_TRY((launch_class<1, 1, false>(ctx, mode, P, grid, st)));
+    else SPARC_TRY((launch_class<2, 1, true>(ctx, mode, P, grid, st)));
+    return SPARC_GPU_SUCCESS;
+}

@@ -99,20 +99,31 @@ def test_h_apply_and_filter_small(torch, api, wl, path):
     g.close()
 
 
-@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("mode", [0, 1, 2, 3])
 def test_nonlocal_modes(torch, api, mode):
-    """Both nonlocal paths (0: fused per-atom kernel with atomic scatter, 1: project + pull, deterministic) against
-    the oracle, on heavily overlapping supports, a ragged number of columns and more rows than one shared tile."""
+    """All nonlocal paths (0: auto = brick-tiled DMMA kernel on this grid, 1: project + pull, deterministic, 2: fused
+    per-atom kernel with atomic scatter, 3: brick kernel forced) against the oracle, on heavily overlapping supports,
+    a ragged number of columns, bricks that overhang the grid in y and z, and more rows than one shared tile."""
     pos = np.array([[3.0, 3.1, 3.3], [3.6, 3.0, 2.9], [2.5, 3.4, 3.8], [6.1, 0.2, 0.7], [0.1, 6.0, 6.2]])
     wl = wlmod.make_custom("nlmodes", (24, 18, 20), (0.3, 0.32, 0.31), (0, 0, 1), 37, 3, pos, [9, 4, 1, 9, 9], 2.4,
                            seed=21)
     assert max(np.diff(wl.supp_ptr)) > 512          # several shared-memory tiles per atom
     g = api.SparcGpu(wl)
     g.set_option("nonlocal_mode", mode)
+    assert g.get_info("nl_brick") == 1 and g.get_info("nl_brick_blocks") > 0
     X = wl.psi_columns(range(wl.ns))
     H = orc.Hamiltonian(wl)
     Yg = g.hamiltonian_apply(api.colmajor_from_numpy(X))
     check_col(api.colmajor_to_numpy(Yg), H.apply(X), f"nonlocal_mode {mode} H*Psi")
+    # the nonlocal term alone (Veff = 0 and the stencil cancel in the difference of two applies)
+    g.set_option("nonlocal", 0)
+    Y0 = g.hamiltonian_apply(api.colmajor_from_numpy(X))
+    g.set_option("nonlocal", 1)
+    Vnl_g = api.colmajor_to_numpy(Yg) - api.colmajor_to_numpy(Y0)
+    Vnl_o = H.vnl_apply(X)
+    e = float(np.linalg.norm(Vnl_g - Vnl_o) / np.linalg.norm(Vnl_o))
+    print(f"[parity] nonlocal_mode {mode} V_nl alone: {e:.3e}")
+    assert e <= 1e-12
     Pg = api.colmajor_from_numpy(X)
     g.chebyshev_filter(Pg, 3, wl.a, wl.b, wl.a0, col_block=17)
     check_col(api.colmajor_to_numpy(Pg), H.chebyshev_filter(X, 3, wl.a, wl.b, wl.a0), f"nonlocal_mode {mode} filter")
@@ -120,6 +131,47 @@ def test_nonlocal_modes(torch, api, mode):
         P2 = api.colmajor_from_numpy(X)
         g.chebyshev_filter(P2, 3, wl.a, wl.b, wl.a0, col_block=17)
         assert torch.equal(P2, Pg)
+    g.close()
+
+
+@pytest.mark.parametrize("nx", [32, 24, 20, 14])
+@pytest.mark.parametrize("projs", [[4, 1, 3], [9, 4, 5]])
+def test_brick_shapes_and_classes(torch, api, nx, projs):
+    """Brick kernel on every brick shape (16x4x4, 8x8x4, 4x8x8, 2x16x8), both projector classes (P <= 4: one DMMA
+    k-step; P <= 9: two k-steps + rank-1 update), Dirichlet and periodic faces, against the oracle and the per-atom
+    deterministic path."""
+    pos = np.array([[0.3, 2.0, 3.0], [4.1, 4.4, 0.2], [2.2, 0.1, 5.9]])
+    wl = wlmod.make_custom(f"brick{nx}", (nx, 14, 19), (0.31, 0.4, 0.35), (0, 1, 0), 11, 4, pos, projs, 2.0, seed=5)
+    g = api.SparcGpu(wl)
+    assert g.get_info("nl_brick") == 1
+    g.set_option("nonlocal_mode", 3)
+    X = wl.psi_columns(range(wl.ns))
+    H = orc.Hamiltonian(wl)
+    Yg = g.hamiltonian_apply(api.colmajor_from_numpy(X))
+    check_col(api.colmajor_to_numpy(Yg), H.apply(X), f"brick nx={nx} P={projs} H*Psi")
+    for m, cb in ((1, 0), (4, 5)):
+        Pg = api.colmajor_from_numpy(X)
+        g.chebyshev_filter(Pg, m, wl.a, wl.b, wl.a0, col_block=cb)
+        check_col(api.colmajor_to_numpy(Pg), H.chebyshev_filter(X, m, wl.a, wl.b, wl.a0), f"brick nx={nx} filter m={m}")
+    g.close()
+
+
+def test_brick_many_atoms_per_brick(torch, api):
+    """More (brick, atom) jobs per brick than the kernel keeps in flight (16 slots, 32-job descriptor batches), so
+    that the producer warp wraps its slots and its byte ring; 70 columns = one full and one ragged column group."""
+    rng = np.random.default_rng(3)
+    pos = rng.uniform(0.0, 4.8, size=(24, 3))
+    wl = wlmod.make_custom("dense_atoms", (16, 16, 16), (0.3, 0.3, 0.3), (0, 0, 0), 70, 3, pos, [9] * 24, 2.0, seed=8)
+    g = api.SparcGpu(wl)
+    assert g.get_info("nl_brick") == 1
+    g.set_option("nonlocal_mode", 3)
+    X = wl.psi_columns(range(wl.ns))
+    H = orc.Hamiltonian(wl)
+    Yg = g.hamiltonian_apply(api.colmajor_from_numpy(X))
+    check_col(api.colmajor_to_numpy(Yg), H.apply(X), "dense atoms H*Psi")
+    Pg = api.colmajor_from_numpy(X)
+    g.chebyshev_filter(Pg, 3, wl.a, wl.b, wl.a0)
+    check_col(api.colmajor_to_numpy(Pg), H.chebyshev_filter(X, 3, wl.a, wl.b, wl.a0), "dense atoms filter m=3")
     g.close()
 
 
