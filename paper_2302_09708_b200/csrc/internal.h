@@ -29,7 +29,7 @@ struct CoverEntry {
 struct NlBrick {
     int ok = 0;                // 0: grid does not meet the preconditions, per-atom kernels are used
     int pclass = 0;            // 4 or 9: projector-count class the blocks are laid out for
-    int bx = 0, by = 0, bz = 0;   // brick shape, bx * by * bz = 256
+    int bx = 0, by = 0, bz = 0;   // brick shape, bx * by * bz = 128
     int32_t n_active = 0;      // bricks met by at least one support
     int64_t n_blocks = 0;      // chi blocks = touched (brick, atom, octet) triples
     int32_t *d_org = nullptr;      // [n_active][4]: x0, y0, z0, union octet mask

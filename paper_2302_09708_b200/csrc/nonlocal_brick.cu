@@ -3,8 +3,8 @@
 //   V_nl X = sum_J S_J^T chi_J diag(gamma_J) chi_J^T S_J X
 //
 // The per-atom formulation gathers X at each atom's support and scatter-adds with atomics: 8c + 16c bytes and one
-// atomic per (support row, column) (c = coverage, 4-5 at configs 3-4).  Here the grid is cut into bricks of 256
-// points (BX x BY x BZ, x fastest) and one CTA owns (brick, 64 columns): it reads the 256 x 64 tile of Out once into
+// atomic per (support row, column) (c = coverage, 4-5 at configs 3-4).  Here the grid is cut into bricks of 128
+// points (BX x BY x BZ, x fastest) and one CTA owns (brick, 64 columns): it reads the 128 x 64 tile of Out once into
 // tensor-core accumulator fragments, adds the contribution of EVERY atom whose support meets the brick
 // ("pull": Out^T[col, pt] += D_J^T[col, q] chi_J^T[q, pt], DMMA m8n8k4), writes the tile back once, and -- the tile
 // now being the final Psi_{k+1} -- contracts it with the same chi blocks for the NEXT degree step
@@ -12,16 +12,15 @@
 // of Out per degree step and one atomic per (brick, atom, projector, column).  The accumulator fragment of the pull
 // is, register for register, the B operand of the projection (k index = point pair), so no layout change is needed.
 //
-// Tables built at create (host): for every (brick, atom) pair a 32-bit mask of the brick's 8-point octets the atom
+// Tables built at create (host): for every (brick, atom) pair a 16-bit mask of the brick's 8-point octets the atom
 // touches, and per touched octet a dense block of chi values already permuted into DMMA fragment order (zeros where
 // the atom does not cover a point; gamma folded into the pull blocks).  Blocks of one (brick, atom) pair are
 // contiguous; a producer warp streams them (and the 64-column slice of C_J) into a shared-memory byte ring with
-// cp.async.bulk, up to 16 (brick, atom) jobs ahead of the eight consumer warps (full / empty mbarriers).
+// cp.async.bulk, up to 16 (brick, atom) jobs ahead of the eight consumer warps; two CTAs share an SM (full / empty mbarriers).
 //
 // The 9th projector of an s+p+d atom is applied as a rank-1 FMA update beside the two k-steps of DMMA (a third
 // k-step would be 3/4 padding).
 #include <algorithm>
-#include <cstdio>
 #include <unordered_map>
 #include <vector>
 
@@ -29,10 +28,9 @@
 
 namespace {
 
-constexpr int NB_PTS = 256;        // points per brick
-constexpr int NB_OCT = 32;         // octets per brick (bit mask width)
-constexpr int NLB_WARPS = 16;      // consumer warps: 8 column slices x 2 brick halves
-constexpr int NB_HOCT = 16;        // octets per brick half (one consumer warp's share)
+constexpr int NB_PTS = 128;        // points per brick
+constexpr int NB_HOCT = 16;        // octets per brick (bit mask width): one consumer warp holds all of them
+constexpr int NLB_WARPS = 8;       // consumer warps: 8 column slices of 8 columns
 constexpr int NLB_COLS = 64;       // columns per CTA: 8 per warp
 
 struct BrickJob {                  // one (brick, atom) pair
@@ -110,16 +108,17 @@ __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
 }
 
 constexpr int NLB_SLOTS = 16;                 // jobs in flight (mbarrier pairs)
-constexpr int NLB_RING_BYTES = 160 * 1024;    // byte ring the producer warp streams chi blocks (+ C slices) through
+constexpr int NLB_RING_BYTES = 72 * 1024;     // byte ring the producer warp streams chi blocks (+ C slices) through
 
 // KP: DMMA k-steps of the pull (projectors 0 .. 4 KP - 1); MT: 8-projector m-tiles of the projection; R1: projector
 // number 8 applied as a rank-1 FMA update (s+p+d atoms: P = 9).  DO_PULL / DO_PROJ select the three variants:
 // project only (C_0 of a filter call, first half of H X), pull only (last degree step, second half of H X), both.
-// Warps 0-15 are consumers (8 columns x one half of the brick each), warp 16 is the producer: it walks the brick's job list ahead of the
+// Warps 0-7 are consumers (8 columns each, the whole 128-point brick), warp 8 is the producer (two CTAs share an SM, so one
+// CTA's tile load / store overlaps the other's DMMAs): it walks the brick's job list ahead of the
 // consumers and streams, per (brick, atom) job, the chi blocks (and for a pull job the 64-column slice of C_J) into a
 // byte ring with cp.async.bulk; full/empty mbarriers per slot.
 template <int KP, int MT, bool R1, bool DO_PULL, bool DO_PROJ>
-__global__ void __launch_bounds__((NLB_WARPS + 1) * 32, 1)
+__global__ void __launch_bounds__((NLB_WARPS + 1) * 32, 2)
 nl_brick_kernel(const BrickParams p)
 {
     constexpr int PULL_SZ = KP * 32 + (R1 ? 8 : 0);
@@ -129,11 +128,8 @@ nl_brick_kernel(const BrickParams p)
     int32_t *pt_off = reinterpret_cast<int32_t *>(ring + NLB_RING_BYTES);             // [NB_PTS] grid index, -1 outside
     uint64_t *full = reinterpret_cast<uint64_t *>(pt_off + NB_PTS);                   // [NLB_SLOTS]
     uint64_t *empty = full + NLB_SLOTS;                                               // [NLB_SLOTS]
-    int32_t *slot_off = reinterpret_cast<int32_t *>(empty + NLB_SLOTS);               // [NLB_SLOTS] ring offset of the job
-    uint32_t *slot_mask = reinterpret_cast<uint32_t *>(slot_off + NLB_SLOTS);         // [NLB_SLOTS]
-    int32_t *slot_pj = reinterpret_cast<int32_t *>(slot_mask + NLB_SLOTS);            // [NLB_SLOTS] P_J
-    int32_t *slot_po = slot_pj + NLB_SLOTS;                                           // [NLB_SLOTS] projector offset of J
-    int32_t *slot_size = slot_po + NLB_SLOTS;                                         // [NLB_SLOTS] ring bytes (producer only)
+    int4 *slot_info = reinterpret_cast<int4 *>(empty + NLB_SLOTS);                    // [NLB_SLOTS] offset, mask, P_J, po
+    int32_t *slot_size = reinterpret_cast<int32_t *>(slot_info + NLB_SLOTS);          // [NLB_SLOTS] ring bytes (producer only)
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int lq = lane & 3, lr = lane >> 2;
@@ -186,12 +182,9 @@ nl_brick_kernel(const BrickParams p)
                 }
                 if (wrap) head = 0;
                 const int slot = jj % NLB_SLOTS;
-#ifdef NLB_DEBUG
-                if (na >= 17 && cg == 0 && jj >= 13) printf("P b=%d jj=%d slot=%d head=%d need=%d skip=%d used=%d freed=%d mask=%08x pj=%d po=%d blk0=%lld bytes=%u+%u\n", brick, jj, slot, head, need, skip, used, freed, mask, pj, po, blk0, blk_bytes, c_bytes);
-#endif
                 slot_size[slot] = need + skip;
                 used += need + skip;
-                slot_off[slot] = head; slot_mask[slot] = mask; slot_pj[slot] = pj; slot_po[slot] = po;
+                slot_info[slot] = make_int4(head, (int)mask, pj, po);
                 mbar_expect_tx(&full[slot], blk_bytes + c_bytes);
                 const double *src = pull ? p.blk_pull + blk0 * PULL_SZ : p.blk_proj + blk0 * PROJ_SZ;
                 bulk_g2s(ring + head, src, blk_bytes, &full[slot]);
@@ -205,14 +198,13 @@ nl_brick_kernel(const BrickParams p)
     }
 
     // ==================================== consumer warps ============================================================
-    // the 128 x 8 tile of this warp (octets 16 half .. 16 half + 15), in accumulator-fragment order: lane (lr, lq)
+    // the 128 x 8 tile of this warp, in accumulator-fragment order: lane (lr, lq)
     // holds column colw + lr, points 2 lq and 2 lq + 1 of every octet
-    const int half = warp >> 3;
     const int colw = cg * NLB_COLS + (warp & 7) * 8;
     const int col = colw + lr;
     const bool colv = col < p.ncols;
-    const uint32_t umask_h = (umask >> (16 * half)) & 0xffffu;
-    const int32_t *pt_h = pt_off + 128 * half + 2 * lq;
+    const uint32_t umask_h = umask & 0xffffu;
+    const int32_t *pt_h = pt_off + 2 * lq;
     const double *srcc = p.src + (int64_t)(colv ? col : 0) * p.ld;
     double2 c[NB_HOCT];
 #pragma unroll
@@ -228,14 +220,11 @@ nl_brick_kernel(const BrickParams p)
         const int slot = jj % NLB_SLOTS;
         const bool pull = DO_PULL && jj < na;
         mbar_wait(&full[slot], (uint32_t)((jj / NLB_SLOTS) & 1));
-        const uint32_t mask_all = slot_mask[slot];
-        const uint32_t mask = (mask_all >> (16 * half)) & 0xffffu;
-        const int blk_h = half ? __popc(mask_all & 0xffffu) : 0;          // first block of this half
-        const int PJ = slot_pj[slot], po = slot_po[slot];
-        const double *base = reinterpret_cast<const double *>(ring + slot_off[slot]);
-#ifdef NLB_DEBUG
-        if (na >= 17 && cg == 0 && jj >= 13 && lane == 0 && (warp == 0 || warp == 15)) printf("C b=%d w=%d jj=%d slot=%d off=%d mask=%08x pj=%d po=%d\n", brick, warp, jj, slot, slot_off[slot], mask_all, PJ, po);
-#endif
+        const int4 info = slot_info[slot];                 // ring offset, octet mask, P_J, projector offset
+        const uint32_t mask_all = (uint32_t)info.y;
+        const uint32_t mask = mask_all & 0xffffu;
+        const int PJ = info.z, po = info.w;
+        const double *base = reinterpret_cast<const double *>(ring + info.x);
 
         if (pull) {
             // A operand: D_J^T[col, q] = scale (chi_J^T Psi_k)[q, col]   (gamma_q is folded into the pull blocks)
@@ -247,19 +236,31 @@ nl_brick_kernel(const BrickParams p)
                 dA[ks] = (q < PJ && (!R1 || q < 8)) ? p.scale * cs[q] : 0.0;
             }
             if (R1) d8 = (8 < PJ) ? p.scale * cs[8] : 0.0;
-            int blk = blk_h;
+            // operands of the next block are fetched while the current block's DMMAs issue (reading one block past
+            // the job's last stays inside the ring / the C slice)
+            const double *bp = base;
+            double nb[KP];
+            double2 nx8 = make_double2(0.0, 0.0);
+#pragma unroll
+            for (int ks = 0; ks < KP; ++ks) nb[ks] = bp[ks * 32 + lane];
+            if (R1) nx8 = *reinterpret_cast<const double2 *>(bp + KP * 32 + 2 * lq);
 #pragma unroll
             for (int o = 0; o < NB_HOCT; ++o) {
                 if (mask & (1u << o)) {
-                    const double *b = base + blk * PULL_SZ;
+                    double b[KP];
 #pragma unroll
-                    for (int ks = 0; ks < KP; ++ks) dmma884(c[o].x, c[o].y, dA[ks], b[ks * 32 + lane]);
+                    for (int ks = 0; ks < KP; ++ks) b[ks] = nb[ks];
+                    const double2 x8 = nx8;
+                    bp += PULL_SZ;
+#pragma unroll
+                    for (int ks = 0; ks < KP; ++ks) nb[ks] = bp[ks * 32 + lane];
+                    if (R1) nx8 = *reinterpret_cast<const double2 *>(bp + KP * 32 + 2 * lq);
+#pragma unroll
+                    for (int ks = 0; ks < KP; ++ks) dmma884(c[o].x, c[o].y, dA[ks], b[ks]);
                     if (R1) {
-                        const double2 x8 = *reinterpret_cast<const double2 *>(b + KP * 32 + 2 * lq);
                         c[o].x = fma(d8, x8.x, c[o].x);
                         c[o].y = fma(d8, x8.y, c[o].y);
                     }
-                    ++blk;
                 }
             }
             __syncwarp();
@@ -283,22 +284,32 @@ nl_brick_kernel(const BrickParams p)
 #pragma unroll
                 for (int mt = 0; mt < MT; ++mt) acc[s][mt][0] = acc[s][mt][1] = 0.0;
             }
-            int blk = blk_h;
+            const double *bp = base;
+            double nb[2 * MT];
+            double2 nx8 = make_double2(0.0, 0.0);
+#pragma unroll
+            for (int k = 0; k < 2 * MT; ++k) nb[k] = bp[k * 32 + lane];
+            if (R1) nx8 = *reinterpret_cast<const double2 *>(bp + MT * 64 + 2 * lq);
 #pragma unroll
             for (int o = 0; o < NB_HOCT; ++o) {
                 if (mask & (1u << o)) {
-                    const double *b = base + blk * PROJ_SZ;
+                    double b[2 * MT];
+#pragma unroll
+                    for (int k = 0; k < 2 * MT; ++k) b[k] = nb[k];
+                    const double2 x8 = nx8;
+                    bp += PROJ_SZ;
+#pragma unroll
+                    for (int k = 0; k < 2 * MT; ++k) nb[k] = bp[k * 32 + lane];
+                    if (R1) nx8 = *reinterpret_cast<const double2 *>(bp + MT * 64 + 2 * lq);
 #pragma unroll
                     for (int mt = 0; mt < MT; ++mt) {
-                        dmma884(acc[o & 1][mt][0], acc[o & 1][mt][1], b[(2 * mt) * 32 + lane], c[o].x);
-                        dmma884(acc[o & 1][mt][0], acc[o & 1][mt][1], b[(2 * mt + 1) * 32 + lane], c[o].y);
+                        dmma884(acc[o & 1][mt][0], acc[o & 1][mt][1], b[2 * mt], c[o].x);
+                        dmma884(acc[o & 1][mt][0], acc[o & 1][mt][1], b[2 * mt + 1], c[o].y);
                     }
                     if (R1) {
-                        const double2 x8 = *reinterpret_cast<const double2 *>(b + MT * 64 + 2 * lq);
                         p8[o & 1] = fma(x8.x, c[o].x, p8[o & 1]);
                         p8[o & 1] = fma(x8.y, c[o].y, p8[o & 1]);
                     }
-                    ++blk;
                 }
             }
             __syncwarp();
@@ -354,10 +365,9 @@ int nlb_build(sparc_gpu_ctx *ctx, const sparc_gpu_desc *d)
     const int nx = ctx->n[0], ny = ctx->n[1], nz = ctx->n[2];
     if (ctx->n_atoms == 0 || ctx->n_proj_total == 0 || ctx->supp_total == 0) return SPARC_GPU_SUCCESS;
     if (ctx->max_proj > 9) return SPARC_GPU_SUCCESS;      // l <= 2 (s+p+d); larger sets use the per-atom kernels
-    if (nx % 16 == 0) { B.bx = 16; B.by = 4; B.bz = 4; }
-    else if (nx % 8 == 0) { B.bx = 8; B.by = 8; B.bz = 4; }
-    else if (nx % 4 == 0) { B.bx = 4; B.by = 8; B.bz = 8; }
-    else if (nx % 2 == 0) { B.bx = 2; B.by = 16; B.bz = 8; }
+    if (nx % 8 == 0) { B.bx = 8; B.by = 4; B.bz = 4; }
+    else if (nx % 4 == 0) { B.bx = 4; B.by = 8; B.bz = 4; }
+    else if (nx % 2 == 0) { B.bx = 2; B.by = 8; B.bz = 8; }
     else return SPARC_GPU_SUCCESS;
     B.pclass = ctx->max_proj <= 4 ? 4 : 9;
     const ClassInfo ci = class_info(B.pclass);
