@@ -35,8 +35,8 @@ UNIT = "grid-pt*orbital*degree/s"
 ALG_BYTES_PER_UNIT = 24.0       # read Psi_k, read Psi_{k-1}, write Psi_{k+1}
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` capture (profiles/r01_ncu_stencil_tma_cfg1.md).  None until captured.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {1: None}
+# `ncu --set full` capture (profiles/r01b_ncu_stencil_tma_cfg1.md), keyed by (config, kernel).
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {(1, "stencil"): 697.6e6}
 
 
 def measured_peaks():
@@ -246,36 +246,75 @@ def run_ours(args):
     e2e_s = float(te.cpu()[0])
     del host_in, host_out
 
-    # ---- roofline of the dominant kernel: per-launch CUDA events inside the library, same launch config ------
+    # ---- rooflines: per-launch CUDA events inside the library (option "profile"), same launch configuration ----
+    # One profiled pass of the whole step (filter, project, rotate) repeated twice; every kernel gets its algorithmic
+    # work per launch over its average launch duration; `roofline` is the kernel with the
+    # largest share of the step, `roofline_by_kernel` lists the others.
     roofline = None
+    rooflines = {}
     kinds = {0: "stencil_generic", 1: "stencil_tma", 2: "nl_project", 3: "nl_pull", 4: "gemm_tn", 5: "gemm_nn",
              6: "splitk_reduce", 7: "copy2d", 8: "nl_fused", 9: "nl_brick"}
     share = {}
     if rank == 0:
+        reps = 2
         g.set_option("profile_reset", 1)
         g.set_option("profile", 1)
-        for _ in range(2):
+        for _ in range(reps):
             refill()
             g.chebyshev_filter(psi, m, wl.a, wl.b, wl.a0, col_block=col_block)
         torch.cuda.synchronize()
+        prof_f = {k: (g.get_info(f"prof_ns:{k}"), g.get_info(f"prof_count:{k}")) for k in kinds}
+        g.set_option("profile_reset", 1)
+        for _ in range(reps):
+            g.project(psi, col_block=col_block, Hs=Hs, Ms=Ms)
+            g.rotate(psi, Q)
+        torch.cuda.synchronize()
         g.set_option("profile", 0)
-        prof = {k: (g.get_info(f"prof_ns:{k}"), g.get_info(f"prof_count:{k}")) for k in kinds}
-        tot = sum(v[0] for v in prof.values()) or 1
-        share = {kinds[k]: round(v[0] / tot, 4) for k, v in prof.items() if v[1]}
-        sk = 1 if prof[1][1] else 0
-        ns_total, n_launch = prof[sk]
-        cb = col_block if col_block and col_block > 0 else min(ns, 1024)
-        nblocks = (ns + cb - 1) // cb
-        # per filter call: each column block launches 1 kernel without Prev (16 B/pt) and m-1 with Prev (24 B/pt)
-        alg_bytes = 2 * nd * ns * (16.0 + 24.0 * (m - 1))
-        achieved = alg_bytes / (ns_total * 1e-9) / 1e9 if ns_total else 0.0
-        peak, peak_src = measured_peaks()
-        traffic = NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.config)
-        roofline = {"bound": "hbm", "kernel": kinds[sk], "achieved": achieved, "peak": peak, "unit": "GB/s",
-                    "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                    "launches_timed": n_launch, "avg_launch_us": ns_total / max(n_launch, 1) / 1e3,
-                    "alg_bytes_per_launch": alg_bytes / max(n_launch, 1),
-                    "filter_time_share_by_kernel": share}
+        prof_s = {k: (g.get_info(f"prof_ns:{k}"), g.get_info(f"prof_count:{k}")) for k in kinds}
+        tot_f = sum(v[0] for v in prof_f.values()) or 1
+        share = {kinds[k]: round(v[0] / tot_f, 4) for k, v in prof_f.items() if v[1]}
+        tot_step = tot_f + (sum(v[0] for v in prof_s.values()) or 0)
+        hbm_peak, hbm_src = measured_peaks()
+        dfma_peak = api.probe_peak(0, local_rank)       # TFLOP/s, register-resident DFMA chains, measured now
+        dmma_peak = api.probe_peak(1, local_rank)       # TFLOP/s, register-resident DMMA.8x8x4 chains
+        supp_rows = float(wl.supp_idx.shape[0])
+        pbar = float(wl.chi.shape[0]) / max(supp_rows, 1.0)          # mean projectors per support row
+
+        def entry(name, bound, ns_total, n_launch, work_total, peak, unit, src, traffic=None, note=None):
+            if not n_launch or not ns_total:
+                return None
+            ach = work_total / (ns_total * 1e-9) / (1e9 if unit == "GB/s" else 1e12)
+            e = {"bound": bound, "kernel": name, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak,
+                 "traffic": traffic, "peak_source": src, "launches_timed": n_launch,
+                 "avg_launch_us": ns_total / n_launch / 1e3, "alg_work_per_launch": work_total / n_launch,
+                 "share_of_step": round(ns_total / tot_step, 4)}
+            if note:
+                e["note"] = note
+            return e
+
+        sk = 1 if prof_f[1][1] else 0
+        # stencil: each column block launches 1 kernel without Prev (16 B/pt) and m-1 with Prev (24 B/pt) per call
+        rooflines["stencil"] = entry(kinds[sk], "hbm", prof_f[sk][0], prof_f[sk][1],
+                                     reps * nd * ns * (16.0 + 24.0 * (m - 1)), hbm_peak, "GB/s", hbm_src,
+                                     traffic=NCU_TRAFFIC_BYTES_PER_LAUNCH.get((args.config, "stencil")))
+        # nonlocal: 2 flop x P x (pull + project) per (support row, column) and degree step; the first pass projects
+        # only, the last pulls only: (2m) half-passes + ... = 2m half-passes per filter call
+        nlk = 9 if prof_f[9][1] else (8 if prof_f[8][1] else None)
+        if nlk is not None:
+            rooflines["nonlocal"] = entry(kinds[nlk], "tensor" if nlk == 9 else "alu", prof_f[nlk][0], prof_f[nlk][1],
+                                          reps * 2.0 * m * 2.0 * supp_rows * pbar * ns,
+                                          dmma_peak if nlk == 9 else dfma_peak, "TFLOP/s",
+                                          "measured now (sparc_gpu_probe_peak, FP64 %s)" % ("DMMA" if nlk == 9 else "DFMA"),
+                                          note="algorithmic flop 4*c*P per pt*orb*deg; padding flop of partial octets not counted")
+        # GEMMs: 2*Nd*Ns^2 flop per product; project = Hs (by column blocks) + Ms, rotate = Psi Q
+        rooflines["gemm_tn"] = entry("gemm_tn", "tensor", prof_s[4][0], prof_s[4][1], reps * 2 * 2.0 * nd * ns * ns,
+                                     dmma_peak, "TFLOP/s", "measured now (sparc_gpu_probe_peak, FP64 DMMA)")
+        rooflines["gemm_nn"] = entry("gemm_nn", "tensor", prof_s[5][0], prof_s[5][1], reps * 2.0 * nd * ns * ns,
+                                     dmma_peak, "TFLOP/s", "measured now (sparc_gpu_probe_peak, FP64 DMMA)")
+        rooflines = {k: v for k, v in rooflines.items() if v}
+        roofline = dict(max(rooflines.values(), key=lambda e: e["share_of_step"]))
+        roofline["filter_time_share_by_kernel"] = share
+        roofline["fp64_peaks_tflops"] = {"dfma": dfma_peak, "dmma": dmma_peak}
 
     # ---- CPU oracle beside it (rank 0, N = 1 only) --------------------------------------------------------
     cpu_baseline = None
@@ -314,6 +353,7 @@ def run_ours(args):
                     "what": "pinned host Psi -> H2D -> sparc_gpu_chebyshev_filter -> D2H, wall clock"},
             "gpu_launches": int(launches),
             "roofline": roofline,
+            "roofline_by_kernel": rooflines,
             "cpu_baseline": cpu_baseline,
         }
         print(json.dumps(line))

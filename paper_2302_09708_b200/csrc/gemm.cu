@@ -12,10 +12,12 @@
 
 namespace {
 
-constexpr int BM = 128, BN = 128, BK = 16, STAGES = 3;
+constexpr int BM = 128, BK = 16, STAGES = 3;
+// CTA tile 128 x (32 NWN): 2 x NWN warps of 64 x 32.  NWN = 2 (128 x 64, 128 threads) lets two CTAs share an SM so that
+// one CTA's pipeline barriers are covered by the other's DMMAs; NWN = 4 is the 128 x 128 tile.
+constexpr int NWN_DEFAULT = 2;
 constexpr int PITCH_K = BK + 4;     // rows of BK doubles (k contiguous)
 constexpr int PITCH_M = BM + 4;     // rows of BM doubles (m contiguous)
-constexpr int GEMM_THREADS = 256;
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem, int src_bytes)
 {
@@ -38,15 +40,15 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
                  : "d"(a), "d"(b));
 }
 
-constexpr size_t smem_bytes(bool a_mmajor)
+constexpr size_t smem_bytes(bool a_mmajor, int nwn)
 {
-    return (size_t)STAGES * ((a_mmajor ? BK * PITCH_M : BM * PITCH_K) + BN * PITCH_K) * sizeof(double);
+    return (size_t)STAGES * ((a_mmajor ? BK * PITCH_M : BM * PITCH_K) + 32 * nwn * PITCH_K) * sizeof(double);
 }
 
 // Load a tile whose contiguous global direction is "inner" (length INNER doubles per row, ROWS rows).
 // Global element (inner i, row r) lives at g[i + r*ld]; rows beyond `rows_valid` and inner beyond
 // `inner_valid` are zero-filled.  Shared layout: s[r*PITCH + i].
-template <int ROWS, int INNER, int PITCH, bool VEC16>
+template <int ROWS, int INNER, int PITCH, bool VEC16, int GEMM_THREADS>
 __device__ __forceinline__ void load_tile(double *s, const double *g, int64_t ld, int64_t rows_valid,
                                           int64_t inner_valid, int tid)
 {
@@ -73,19 +75,20 @@ __device__ __forceinline__ void load_tile(double *s, const double *g, int64_t ld
 // A_MMAJOR = true : A is M x K col-major (A[m + k*lda]) -> C = A B             (NN)
 // B is always K x N col-major (B[k + n*ldb]).  C is M x N col-major; with splits > 1, blockIdx.z writes its
 // partial product to Cpart + z*M*N (ld = M).
-template <bool A_MMAJOR, bool VEC16>
-__global__ void __launch_bounds__(GEMM_THREADS, 1)
+template <bool A_MMAJOR, bool VEC16, int NWN>
+__global__ void __launch_bounds__(64 * NWN, NWN == 2 ? 2 : 1)
 gemm_dmma_kernel(const double *__restrict__ A, int64_t lda, const double *__restrict__ B, int64_t ldb, double *C,
                  int64_t ldc, int64_t M, int64_t N, int64_t K, int64_t k_chunk, int tiles_m)
 {
     extern __shared__ __align__(16) double smem[];
+    constexpr int BN = 32 * NWN, GEMM_THREADS = 64 * NWN;
     constexpr int A_STAGE = A_MMAJOR ? BK * PITCH_M : BM * PITCH_K;
     constexpr int B_STAGE = BN * PITCH_K;
     double *As = smem;
     double *Bs = smem + STAGES * A_STAGE;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int wm = warp >> 2, wn = warp & 3;          // 2 x 4 warps, warp tile 64 x 32
+    const int wm = warp / NWN, wn = warp % NWN;       // 2 x NWN warps, warp tile 64 x 32
     const int tile_m = blockIdx.x % tiles_m, tile_n = blockIdx.x / tiles_m;
     const int64_t m0 = (int64_t)tile_m * BM, n0 = (int64_t)tile_n * BN;
     const int64_t k_begin = (int64_t)blockIdx.z * k_chunk;
@@ -104,10 +107,10 @@ gemm_dmma_kernel(const double *__restrict__ A, int64_t lda, const double *__rest
         const int64_t k0 = k_begin + (int64_t)kt * BK;
         const int64_t kv = k_end - k0;      // valid k in this tile (may exceed BK)
         if (A_MMAJOR)
-            load_tile<BK, BM, PITCH_M, VEC16>(As + s * A_STAGE, A + m0 + k0 * lda, lda, kv, M - m0, tid);
+            load_tile<BK, BM, PITCH_M, VEC16, GEMM_THREADS>(As + s * A_STAGE, A + m0 + k0 * lda, lda, kv, M - m0, tid);
         else
-            load_tile<BM, BK, PITCH_K, VEC16>(As + s * A_STAGE, A + k0 + m0 * lda, lda, M - m0, kv, tid);
-        load_tile<BN, BK, PITCH_K, VEC16>(Bs + s * B_STAGE, B + k0 + n0 * ldb, ldb, N - n0, kv, tid);
+            load_tile<BM, BK, PITCH_K, VEC16, GEMM_THREADS>(As + s * A_STAGE, A + k0 + m0 * lda, lda, M - m0, kv, tid);
+        load_tile<BN, BK, PITCH_K, VEC16, GEMM_THREADS>(Bs + s * B_STAGE, B + k0 + n0 * ldb, ldb, N - n0, kv, tid);
     };
 
 #pragma unroll
@@ -186,8 +189,9 @@ struct SplitPlan { int splits; int64_t k_chunk; };
 // workspace and are summed in a fixed order (deterministic).
 SplitPlan plan_tn(const sparc_gpu_ctx *ctx, int64_t M, int64_t N, int64_t K)
 {
+    const int BN = 32 * NWN_DEFAULT;
     const int64_t tiles = ((M + BM - 1) / BM) * ((N + BN - 1) / BN);
-    const int64_t sms = std::max(1, ctx->sm_count);
+    const int64_t sms = std::max(1, ctx->sm_count) * (NWN_DEFAULT == 2 ? 2 : 1);      // CTA slots
     const int64_t max_splits = std::max<int64_t>(1, std::min<int64_t>(64, K / (16 * BK)));
     const int64_t ws_cap = (int64_t)2 << 30;                       // at most 2 GiB of partial products
     int64_t best_s = 1;
@@ -213,18 +217,19 @@ template <bool A_MMAJOR>
 int launch_dmma(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const double *B, int64_t ldb, double *C, int64_t ldc,
                 int64_t M, int64_t N, int64_t K, SplitPlan plan, cudaStream_t st)
 {
+    constexpr int NWN = NWN_DEFAULT, BN = 32 * NWN, GEMM_THREADS = 64 * NWN;
     const int tiles_m = (int)((M + BM - 1) / BM), tiles_n = (int)((N + BN - 1) / BN);
     dim3 grid((unsigned)(tiles_m * tiles_n), 1, (unsigned)plan.splits);
     const bool vec = aligned16(A) && aligned16(B) && (lda % 2 == 0) && (ldb % 2 == 0);
-    const size_t smem = smem_bytes(A_MMAJOR);
+    const size_t smem = smem_bytes(A_MMAJOR, NWN);
     const int kind = A_MMAJOR ? KK_GEMM_NN : KK_GEMM_TN;
     if (vec) {
-        auto kern = gemm_dmma_kernel<A_MMAJOR, true>;
+        auto kern = gemm_dmma_kernel<A_MMAJOR, true, NWN>;
         SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         prof_begin(ctx, kind, st);
         kern<<<grid, GEMM_THREADS, smem, st>>>(A, lda, B, ldb, C, ldc, M, N, K, plan.k_chunk, tiles_m);
     } else {
-        auto kern = gemm_dmma_kernel<A_MMAJOR, false>;
+        auto kern = gemm_dmma_kernel<A_MMAJOR, false, NWN>;
         SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         prof_begin(ctx, kind, st);
         kern<<<grid, GEMM_THREADS, smem, st>>>(A, lda, B, ldb, C, ldc, M, N, K, plan.k_chunk, tiles_m);
