@@ -190,7 +190,9 @@ int local_pass(sparc_gpu_ctx *c, const double *X, int64_t ldx, double *Out, int6
 {
     int path = c->opt_stencil_path;
     if (path == 0) path = stencil_tma_supported(c, X, ldx, Out, ldo, Prev, ldp) ? 2 : 1;
-    if (path == 2) {
+    if (path == 3) {
+        SPARC_TRY(launch_stencil_dmma(c, X, ldx, Out, ldo, Prev, ldp, ncols, alpha, shift, beta, st));
+    } else if (path == 2) {
         SPARC_TRY(launch_stencil_tma(c, X, ldx, Out, ldo, Prev, ldp, ncols, alpha, shift, beta, st));
     } else {
         SPARC_TRY(launch_stencil_generic(c, X, ldx, Out, ldo, Prev, ldp, ncols, alpha, shift, beta, st));
@@ -389,7 +391,7 @@ int sparc_gpu_set_veff(sparc_gpu_ctx *ctx, const double *veff_dev, void *stream)
 int sparc_gpu_set_option(sparc_gpu_ctx *ctx, const char *key, int64_t value)
 {
     if (!ctx || !key) return SPARC_GPU_INVALID_ARG;
-    if (!strcmp(key, "stencil_path")) { if (value < 0 || value > 2) return SPARC_GPU_INVALID_ARG; ctx->opt_stencil_path = (int)value; return 0; }
+    if (!strcmp(key, "stencil_path")) { if (value < 0 || value > 3) return SPARC_GPU_INVALID_ARG; ctx->opt_stencil_path = (int)value; return 0; }
     if (!strcmp(key, "nonlocal_mode")) { if (value < 0 || value > 3) return SPARC_GPU_INVALID_ARG; ctx->opt_nonlocal_mode = (int)value; return 0; }
     if (!strcmp(key, "nonlocal")) { ctx->opt_nonlocal = value ? 1 : 0; return 0; }
     if (!strcmp(key, "profile")) { if (!ctx->prof) return SPARC_GPU_OUT_OF_MEMORY; ctx->prof->on = value != 0; return 0; }

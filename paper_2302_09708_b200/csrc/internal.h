@@ -70,7 +70,7 @@ struct sparc_gpu_ctx {
     // local potential
     double *d_veff;            // [nd]
     // options
-    int opt_stencil_path;      // 0 auto, 1 generic, 2 TMA
+    int opt_stencil_path;      // 0 auto, 1 generic, 2 TMA (DFMA), 3 TMA + DMMA in-plane taps
     int opt_nonlocal;          // 1 on
     int opt_gemm_path;         // 0 auto, 1 simple, 2 DMMA
     int opt_nonlocal_mode;     // 0 auto (brick kernel when supported, else 2), 1 project + pull (deterministic),
@@ -124,6 +124,12 @@ int launch_stencil_generic(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, dou
 int launch_stencil_tma(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double *Out, int64_t ldo,
                        const double *Prev, int64_t ldp, int64_t ncols, double alpha, double shift,
                        double beta, cudaStream_t st);
+// same contract; hybrid kernel: in-plane taps as DMMA, z taps as DFMA (stencil_dmma.cu)
+int launch_stencil_dmma(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double *Out, int64_t ldo,
+                        const double *Prev, int64_t ldp, int64_t ncols, double alpha, double shift,
+                        double beta, cudaStream_t st);
+bool stencil_dmma_supported(const sparc_gpu_ctx *ctx, const double *X, int64_t ldx, const double *Out,
+                            int64_t ldo, const double *Prev, int64_t ldp);
 bool stencil_tma_supported(const sparc_gpu_ctx *ctx, const double *X, int64_t ldx, const double *Out,
                            int64_t ldo, const double *Prev, int64_t ldp);
 

@@ -1,0 +1,388 @@
+// stencil_dmma.cu -- hybrid fused local pass: the in-plane (x, y) taps of the radius-6 stencil on the FP64 tensor pipe,
+// the z taps and the pointwise terms on the FP64 FMA pipe.
+//     Out = alpha (H_loc X + shift X) + beta Prev,   H_loc = -1/2 Laplacian(radius 6) + Veff
+//
+// Same data path as stencil_tma.cu (producer warp, TMA ring of input planes + Veff / Prev tiles, z march with 13 partial
+// sums per point in registers).  What changes is the in-plane part: a warp owns an 8 (y) x 8 (x) block of outputs and
+// evaluates
+//     y taps:  C[y_out, x] += T_y[y_out, y_in] . In[y_in, x]        (A = 8 x 20 banded Toeplitz constants, B = data)
+//     x taps:  C[y, x_out] += In[y, x_in] . T_x[x_in, x_out]        (A = data, B = 20 x 8 banded Toeplitz constants)
+// as 5 + 5 DMMA.8x8x4 with the partial z-sum of the centre plane as accumulator.  Both products leave lane (r, c) of
+// the warp with row y0 + r, columns x0 + 2c, x0 + 2c + 1 -- the two points whose z-sums that lane keeps.  The band is
+// 13 / 20 dense, so the tensor pipe does 1.5 x the arithmetic, but one instruction replaces 8 DFMA-pairs and 8 shared-
+// memory loads per point pair become 10 LDS.64 per 64 points: the DFMA version is bound by instruction latency at 10-11
+// warps per SM (168 registers), not by either pipe (profiles/r01b_ncu_kernels_cfg1.md).
+// Shared-memory row pitch W = 4 or 12 mod 16 doubles: the x-tap fragments (8 rows x 4 consecutive x) are conflict-free,
+// the y-tap fragments (4 rows x 8 consecutive x) 2-way.
+#include <cuda.h>
+
+#include <algorithm>
+
+#include "internal.h"
+
+namespace {
+
+constexpr int R = 6;
+constexpr int NSLOT = 2 * R + 1;
+constexpr int TY = 8;              // tile rows = one DMMA m-tile
+constexpr int KS = 5;              // k-steps of 4 over the 20-wide input window
+constexpr int MAX_STAGES = 8;
+
+struct DmParams {
+    double cx[R + 1], cy[R + 1], cz[R + 1];   // alpha * (-1/2 w_p / h^2)
+    double c0a;                                // alpha * (c0 + shift)
+    double alpha, beta;
+    double *out;
+    int64_t ldo;
+    int nx, ny, nz;
+    int W;            // smem row pitch in doubles (all three tiles)
+    int x_start;      // first x coordinate of the boxes: 0 (periodic x) or -6 (Dirichlet x)
+    int nwarps;       // consumer warps = nx / 8
+    int nstage;
+    int ytiles, zchunks, zchunk_len;
+    int per_x, per_y, per_z;
+    uint32_t psi_bytes, tile_bytes, stage_bytes;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" ::"r"(smem_u32(bar)),
+                 "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "DM_WAIT:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DM_DONE;\n\t"
+        "bra DM_WAIT;\n\t"
+        "DM_DONE:\n\t"
+        "}" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ double lds1(uint32_t addr)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ double2 lds2(uint32_t addr)
+{
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap *tmap, uint64_t *bar, int x, int y, int z, int c)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(
+            dst),
+        "l"(tmap), "r"(x), "r"(y), "r"(z), "r"(c), "r"(smem_u32(bar))
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *tmap, uint64_t *bar, int x, int y, int z)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+            dst),
+        "l"(tmap), "r"(x), "r"(y), "r"(z), "r"(smem_u32(bar))
+        : "memory");
+}
+__device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
+
+template <bool HAS_PREV>
+__global__ void __launch_bounds__(13 * 32, 1)
+stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
+                    const __grid_constant__ CUtensorMap tmap_v, const __grid_constant__ CUtensorMap tmap_p,
+                    const __grid_constant__ DmParams P)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    uint64_t *bar_full = reinterpret_cast<uint64_t *>(smem_raw);    // [MAX_STAGES] TMA landed
+    uint64_t *bar_empty = bar_full + MAX_STAGES;                    // [MAX_STAGES] consumers done
+    const uint32_t stage0 = (smem_u32(smem_raw) + 2 * MAX_STAGES * 8 + 127u) & ~127u;
+
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        for (int s = 0; s < P.nstage; ++s) {
+            mbar_init(&bar_full[s], 1);
+            mbar_init(&bar_empty[s], (uint32_t)P.nwarps);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    const int per_col = P.ytiles * P.zchunks;
+    const int col = blockIdx.x / per_col;
+    const int rem = blockIdx.x - col * per_col;
+    const int ytile = rem / P.zchunks;
+    const int zc = rem - ytile * P.zchunks;
+    const int y0 = ytile * TY;
+    const int z0 = zc * P.zchunk_len;
+    const int z1 = min(z0 + P.zchunk_len, P.nz);
+    const int nzc = z1 - z0;
+    const int nsteps = nzc + 2 * R;          // input planes z0-6 .. z1+5
+    const int W = P.W;
+
+    if (tid < 32) {
+        // ================================ producer warp (one lane) =======================================
+        if (tid != 0) return;
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_x8) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_v) : "memory");
+        if (HAS_PREV) asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_p) : "memory");
+        const uint32_t row_bytes = (uint32_t)(W * 8);
+        const uint32_t tile_tx = (uint32_t)(TY * W * 8);
+        // three 8-row boxes (128-byte aligned destinations): rows y0-8 .. y0-1 (6 used), y0 .. y0+7, y0+8 .. y0+15
+        // (6 used); the halo boxes wrap as a whole on a periodic y axis, rows outside a Dirichlet face are zero-filled
+        int yt = y0 - TY, yb = y0 + TY;
+        if (P.per_y) { if (yt < 0) yt += P.ny; if (yb >= P.ny) yb -= P.ny; }
+        int stage = 0;
+        uint32_t phase = 0;
+        for (int s = 0; s < nsteps; ++s) {
+            if (s >= P.nstage) {
+                while (!mbar_try_wait(&bar_empty[stage], phase ^ 1u)) __nanosleep(40);
+            }
+            const bool do_xy = (s >= R) && (s < R + nzc);
+            const bool do_prev = HAS_PREV && (s >= 2 * R);
+            int zin = z0 - R + s;
+            if (P.per_z) { if (zin < 0) zin += P.nz; else if (zin >= P.nz) zin -= P.nz; }
+            const uint32_t dst = stage0 + (uint32_t)stage * P.stage_bytes;
+            mbar_arrive_expect_tx(&bar_full[stage], P.psi_bytes + (do_xy ? tile_tx : 0u) + (do_prev ? tile_tx : 0u));
+            tma_load_4d(dst, &tmap_x8, &bar_full[stage], P.x_start, yt, zin, col);
+            tma_load_4d(dst + TY * row_bytes, &tmap_x8, &bar_full[stage], P.x_start, y0, zin, col);
+            tma_load_4d(dst + 2 * TY * row_bytes, &tmap_x8, &bar_full[stage], P.x_start, yb, zin, col);
+            if (do_xy) tma_load_3d(dst + P.psi_bytes, &tmap_v, &bar_full[stage], 0, y0, z0 - R + s);
+            if (do_prev) tma_load_4d(dst + P.psi_bytes + P.tile_bytes, &tmap_p, &bar_full[stage], 0, y0, z0 - 2 * R + s, col);
+            if (++stage == P.nstage) { stage = 0; phase ^= 1u; }
+        }
+        return;
+    }
+
+    // ==================================== consumer warps ====================================================
+    const int cw = (tid >> 5) - 1;             // 8-wide x block of this warp
+    if (cw >= P.nwarps) return;
+    const int lane = tid & 31, lq = lane & 3, lr = lane >> 2;
+    const int x0 = 8 * cw;
+    const int xoff = P.per_x ? 0 : R;           // halo columns are stored only for a Dirichlet x axis
+    // Toeplitz fragments: tap distance d = (k - 6) - (output index), k = 4 s + lq; the centre tap is pointwise
+    double ay[KS], bx[KS];
+    uint32_t xa[KS];                            // byte offsets of the x-tap data fragments (row y0 + lr, wrapped column)
+#pragma unroll
+    for (int s = 0; s < KS; ++s) {
+        const int d = 4 * s + lq - R - lr;
+        const int ad = d < 0 ? -d : d;
+        ay[s] = (ad >= 1 && ad <= R) ? P.cy[ad] : 0.0;
+        bx[s] = (ad >= 1 && ad <= R) ? P.cx[ad] : 0.0;
+        int xc = x0 - R + 4 * s + lq;
+        if (P.per_x) { if (xc < 0) xc += P.nx; else if (xc >= P.nx) xc -= P.nx; }
+        else xc += R;
+        xa[s] = (uint32_t)(((TY + lr) * W + xc) * 8);
+    }
+    const uint32_t ya0 = (uint32_t)(((TY - R + lq) * W + x0 + lr + xoff) * 8);      // row y0 - 6 + lq, + s * 4 rows
+    const uint32_t ystep = (uint32_t)(4 * W * 8);
+    const uint32_t own_off = (uint32_t)(((TY + lr) * W + x0 + 2 * lq + xoff) * 8);
+    const uint32_t tile_off = P.psi_bytes + (uint32_t)((lr * W + x0 + 2 * lq) * 8);
+    const int64_t plane = (int64_t)P.nx * P.ny;
+    double *out_z = P.out + (int64_t)col * P.ldo + (int64_t)(y0 + lr) * P.nx + x0 + 2 * lq + (int64_t)(z0 - 2 * R) * plane;
+
+    double acc[NSLOT][2];
+#pragma unroll
+    for (int s = 0; s < NSLOT; ++s) acc[s][0] = acc[s][1] = 0.0;
+
+    int s = 0, stage = 0;
+    uint32_t phase = 0;
+    for (int sb = 0; sb < nsteps; sb += NSLOT) {
+#pragma unroll
+        for (int ph = 0; ph < NSLOT; ++ph) {
+            if (s >= nsteps) break;
+            const bool do_xy = (s >= R) && (s < R + nzc);
+            const bool do_store = (s >= 2 * R);
+            const uint32_t st = stage0 + (uint32_t)stage * P.stage_bytes;
+
+            mbar_wait(&bar_full[stage], phase);
+            const double2 own = lds2(st + own_off);
+            // ---- in-plane taps of the plane this one is the centre of: 5 + 5 DMMA into its partial z-sum ------
+            if (do_xy) {
+                double fy[KS], fx[KS];
+#pragma unroll
+                for (int k = 0; k < KS; ++k) {
+                    fy[k] = lds1(st + ya0 + k * ystep);
+                    fx[k] = lds1(st + xa[k]);
+                }
+                const double2 vf = lds2(st + tile_off);
+                // this plane's own slot was opened by the plane six steps back (or is the first use in the chunk)
+                double c0 = acc[ph][0], c1 = acc[ph][1], e0 = 0.0, e1 = 0.0;
+#pragma unroll
+                for (int k = 0; k < KS; ++k) {
+                    dmma884(c0, c1, ay[k], fy[k]);        // y taps: constants x data
+                    dmma884(e0, e1, fx[k], bx[k]);        // x taps: data x constants (second chain)
+                }
+                acc[ph][0] = c0 + fma(fma(P.alpha, vf.x, P.c0a), own.x, e0);
+                acc[ph][1] = c1 + fma(fma(P.alpha, vf.y, P.c0a), own.y, e1);
+            }
+            // ---- z taps: this plane feeds the 12 neighbouring output planes --------------------------------------
+#pragma unroll
+            for (int d = -R; d <= R; ++d) {
+                if (d == 0) continue;
+                const int slot = (ph - d + NSLOT) % NSLOT;
+                const double c = P.cz[d < 0 ? -d : d];
+                if (d == -R) {            // first contribution to output plane zin + 6: opens the slot
+                    acc[slot][0] = c * own.x;
+                    acc[slot][1] = c * own.y;
+                } else {
+                    acc[slot][0] = fma(c, own.x, acc[slot][0]);
+                    acc[slot][1] = fma(c, own.y, acc[slot][1]);
+                }
+            }
+            double2 pv = make_double2(0.0, 0.0);
+            if (HAS_PREV && do_store) pv = lds2(st + tile_off + P.tile_bytes);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bar_empty[stage]);
+            if (++stage == P.nstage) { stage = 0; phase ^= 1u; }
+
+            // ---- output plane zin - 6 has all 37 taps: recurrence axpy + store ---------------------------------
+            if (do_store) {
+                const int cs = (ph + R + 1) % NSLOT;
+                double2 o;
+                o.x = HAS_PREV ? fma(P.beta, pv.x, acc[cs][0]) : acc[cs][0];
+                o.y = HAS_PREV ? fma(P.beta, pv.y, acc[cs][1]) : acc[cs][1];
+                *reinterpret_cast<double2 *>(out_z) = o;
+            }
+            out_z += plane;
+            ++s;
+        }
+    }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// (x, y, z[, column]) tensor map over an N_d x ncols column-major block; box = bx x by x 1 [x 1]
+bool encode_map(const sparc_gpu_ctx *ctx, CUtensorMap *tm, const void *base, int rank, int64_t ncols, int64_t ld, int bx,
+                int by)
+{
+    const int nx = ctx->n[0], ny = ctx->n[1], nz = ctx->n[2];
+    const cuuint64_t gdim[4] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nz, (cuuint64_t)std::max<int64_t>(ncols, 1)};
+    const cuuint64_t gstr[3] = {(cuuint64_t)nx * 8, (cuuint64_t)nx * ny * 8, (cuuint64_t)ld * 8};
+    const cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, 1, 1};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult cr = ((EncodeTiledFn)ctx->fn_encode_tiled)(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, (cuuint32_t)rank, (void *)base,
+                                                        gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                                        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                                                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return cr == CUDA_SUCCESS;
+}
+
+// smallest pitch >= need with pitch mod 16 in {4, 12}: 8 rows x 4 consecutive doubles then tile all 32 banks
+int pick_pitch(int need)
+{
+    int w = need;
+    while (!((w % 16) == 4 || (w % 16) == 12)) ++w;
+    return w;
+}
+
+bool a16(const void *p) { return ((uintptr_t)p & 15) == 0; }
+
+}  // namespace
+
+bool stencil_dmma_supported(const sparc_gpu_ctx *ctx, const double *X, int64_t ldx, const double *Out, int64_t ldo,
+                            const double *Prev, int64_t ldp)
+{
+    if (!ctx->fn_encode_tiled || ctx->radius != R) return false;
+    const int nx = ctx->n[0], ny = ctx->n[1];
+    if (nx % 8 || nx < 16 || nx > 96) return false;          // <= 12 consumer warps
+    if (ny % TY || ny < 2 * TY) return false;
+    if (pick_pitch(ctx->bc[0] == 0 ? nx : nx + 2 * R) > 256) return false;
+    if (!a16(X) || !a16(Out) || (Prev && !a16(Prev)) || (ldx & 1) || (ldo & 1) || (Prev && (ldp & 1))) return false;
+    return true;
+}
+
+int launch_stencil_dmma(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double *Out, int64_t ldo, const double *Prev,
+                        int64_t ldp, int64_t ncols, double alpha, double shift, double beta, cudaStream_t st)
+{
+    const bool has_prev = (beta != 0.0) && Prev;
+    if (!stencil_dmma_supported(ctx, X, ldx, Out, ldo, has_prev ? Prev : nullptr, ldp)) return SPARC_GPU_UNSUPPORTED;
+    const int nx = ctx->n[0], ny = ctx->n[1], nz = ctx->n[2];
+    DmParams P;
+    for (int p = 0; p <= R; ++p) { P.cx[p] = alpha * ctx->coef.cx[p]; P.cy[p] = alpha * ctx->coef.cy[p]; P.cz[p] = alpha * ctx->coef.cz[p]; }
+    P.c0a = alpha * (ctx->coef.c0 + shift);
+    P.alpha = alpha; P.beta = beta;
+    P.ldo = ldo;
+    P.nx = nx; P.ny = ny; P.nz = nz;
+    P.per_x = ctx->bc[0] == 0; P.per_y = ctx->bc[1] == 0; P.per_z = ctx->bc[2] == 0;
+    P.W = pick_pitch(P.per_x ? nx : nx + 2 * R);
+    P.x_start = P.per_x ? 0 : -R;
+    P.nwarps = nx / 8;
+    P.ytiles = ny / TY;
+    P.psi_bytes = (uint32_t)(3 * TY * P.W * 8);
+    P.tile_bytes = (uint32_t)(TY * P.W * 8);
+    P.stage_bytes = P.psi_bytes + 2 * P.tile_bytes;
+    const int threads = (P.nwarps + 1) * 32;
+    auto kern = has_prev ? stencil_dmma_kernel<true> : stencil_dmma_kernel<false>;
+    // ring depth: three stages, more when shared memory is plentiful (one or two CTAs per SM by registers)
+    const int ctas = threads <= 256 ? 2 : 1;
+    int nstage = (int)std::min<int64_t>(ctx->opt_stencil_stages > 0 ? ctx->opt_stencil_stages : 4,
+                                        (227 * 1024 / ctas - 2048) / P.stage_bytes);
+    nstage = std::min(nstage, MAX_STAGES);
+    if (nstage < 2) return SPARC_GPU_UNSUPPORTED;
+    P.nstage = nstage;
+    const size_t smem = 512 + (size_t)nstage * P.stage_bytes;
+    SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+
+    CUtensorMap tmap_v;
+    if (!encode_map(ctx, &tmap_v, ctx->d_veff, 3, 1, ctx->nd, P.W, TY)) return SPARC_GPU_CUDA_ERROR;
+    const int64_t max_cols_per_launch = std::max<int64_t>(1, (int64_t)INT32_MAX / ((int64_t)P.ytiles * nz));
+    for (int64_t j0 = 0; j0 < ncols; j0 += max_cols_per_launch) {
+        const int64_t nb = std::min<int64_t>(max_cols_per_launch, ncols - j0);
+        int zchunks = 1;
+        const int64_t base = nb * P.ytiles;
+        const int64_t want = 2LL * ctx->sm_count * ctas;
+        if (base < want) zchunks = (int)std::min<int64_t>((want + base - 1) / base, std::max(1, nz / 12));
+        if (ctx->opt_stencil_zchunks > 0) zchunks = std::min(ctx->opt_stencil_zchunks, nz);
+        P.zchunk_len = (nz + zchunks - 1) / zchunks;
+        P.zchunks = (nz + P.zchunk_len - 1) / P.zchunk_len;
+        P.out = Out + j0 * ldo;
+        CUtensorMap tmap_x, tmap_p;
+        if (!encode_map(ctx, &tmap_x, X + j0 * ldx, 4, nb, ldx, P.W, TY)) return SPARC_GPU_CUDA_ERROR;
+        if (!encode_map(ctx, &tmap_p, has_prev ? Prev + j0 * ldp : X + j0 * ldx, 4, nb, has_prev ? ldp : ldx, P.W, TY))
+            return SPARC_GPU_CUDA_ERROR;
+        const unsigned grid = (unsigned)(nb * P.ytiles * P.zchunks);
+        prof_begin(ctx, KK_STENCIL_TMA, st);
+        kern<<<grid, threads, smem, st>>>(tmap_x, tmap_v, tmap_p, P);
+        prof_end(ctx, KK_STENCIL_TMA, st);
+    }
+    SPARC_CUDA_TRY(cudaGetLastError());
+    return SPARC_GPU_SUCCESS;
+}
