@@ -134,9 +134,14 @@ int sparc_gpu_fill_uniform(double *dst_dev, int64_t count, uint64_t seed, uint64
 int sparc_gpu_probe_peak(int device, int kind, double *value_out, void *scratch_dev, int64_t scratch_bytes,
                          void *stream);
 
-/* Tuning / test knobs.  key: "stencil_path" (0 auto, 1 generic kernel, 2 TMA kernel or UNSUPPORTED),
- * "nonlocal" (1 on, 0 off: drops V_nl, used by closed-form pins), "gemm_path" (0 auto, 1 simple FMA
- * kernel, 2 DMMA kernel).  Unknown key -> INVALID_ARG. */
+/* Tuning / test knobs.  key: "stencil_path" (0 auto, 1 generic kernel, 2 TMA + DFMA kernel, 3 TMA + DMMA in-plane
+ * taps; 2 and 3 return UNSUPPORTED from the operator call when the grid does not meet their preconditions),
+ * "nonlocal" (1 on, 0 off: drops V_nl, used by closed-form pins), "nonlocal_mode" (0 auto = brick-tiled DMMA kernel
+ * when supported, 1 project + pull: bitwise reproducible, 2 per-atom fused kernel with atomic scatter, 3 brick kernel
+ * or UNSUPPORTED), "gemm_path" (0 auto, 1 simple FMA kernel, 2 DMMA kernel), "profile" / "profile_reset" (per-kernel
+ * CUDA-event timing read back through sparc_gpu_get_info "prof_ns:<kind>" / "prof_count:<kind>"), and the stencil
+ * tile knobs "stencil_ay", "stencil_ty", "stencil_stages", "stencil_zchunks" (0 = library chooses).
+ * Unknown key -> INVALID_ARG. */
 int sparc_gpu_set_option(sparc_gpu_ctx *ctx, const char *key, int64_t value);
 
 /* Read-only counters / facts.  key: "kernel_launches" (cumulative kernels launched by this context),

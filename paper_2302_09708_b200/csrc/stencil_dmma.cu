@@ -24,7 +24,7 @@ namespace {
 
 constexpr int R = 6;
 constexpr int NSLOT = 2 * R + 1;
-constexpr int TY = 8;              // tile rows = one DMMA m-tile
+constexpr int TB = 8;              // rows of one DMMA m-tile; a CTA tile has TYB of them (TY = 8 TYB rows)
 constexpr int KS = 5;              // k-steps of 4 over the 20-wide input window
 constexpr int MAX_STAGES = 8;
 
@@ -37,7 +37,8 @@ struct DmParams {
     int nx, ny, nz;
     int W;            // smem row pitch in doubles (all three tiles)
     int x_start;      // first x coordinate of the boxes: 0 (periodic x) or -6 (Dirichlet x)
-    int nwarps;       // consumer warps = nx / 8
+    int nwarps;       // consumer warps = TYB * nx / 8
+    int nxb;          // x blocks = nx / 8
     int nstage;
     int ytiles, zchunks, zchunk_len;
     int per_x, per_y, per_z;
@@ -122,7 +123,7 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
                  : "d"(a), "d"(b));
 }
 
-template <bool HAS_PREV>
+template <bool HAS_PREV, int TYB>
 __global__ void __launch_bounds__(13 * 32, 1)
 stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
                     const __grid_constant__ CUtensorMap tmap_v, const __grid_constant__ CUtensorMap tmap_p,
@@ -133,6 +134,7 @@ stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
     uint64_t *bar_empty = bar_full + MAX_STAGES;                    // [MAX_STAGES] consumers done
     const uint32_t stage0 = (smem_u32(smem_raw) + 2 * MAX_STAGES * 8 + 127u) & ~127u;
 
+    constexpr int TY = TB * TYB;
     const int tid = threadIdx.x;
     if (tid == 0) {
         for (int s = 0; s < P.nstage; ++s) {
@@ -163,9 +165,10 @@ stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
         if (HAS_PREV) asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_p) : "memory");
         const uint32_t row_bytes = (uint32_t)(W * 8);
         const uint32_t tile_tx = (uint32_t)(TY * W * 8);
-        // three 8-row boxes (128-byte aligned destinations): rows y0-8 .. y0-1 (6 used), y0 .. y0+7, y0+8 .. y0+15
-        // (6 used); the halo boxes wrap as a whole on a periodic y axis, rows outside a Dirichlet face are zero-filled
-        int yt = y0 - TY, yb = y0 + TY;
+        // TYB + 2 boxes of 8 rows (128-byte aligned destinations): rows y0-8 .. y0-1 (6 used), the tile, y0+TY ..
+        // y0+TY+7 (6 used); the halo boxes wrap as a whole on a periodic y axis, rows outside a Dirichlet face are
+        // zero-filled
+        int yt = y0 - TB, yb = y0 + TY;
         if (P.per_y) { if (yt < 0) yt += P.ny; if (yb >= P.ny) yb -= P.ny; }
         int stage = 0;
         uint32_t phase = 0;
@@ -180,8 +183,10 @@ stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
             const uint32_t dst = stage0 + (uint32_t)stage * P.stage_bytes;
             mbar_arrive_expect_tx(&bar_full[stage], P.psi_bytes + (do_xy ? tile_tx : 0u) + (do_prev ? tile_tx : 0u));
             tma_load_4d(dst, &tmap_x8, &bar_full[stage], P.x_start, yt, zin, col);
-            tma_load_4d(dst + TY * row_bytes, &tmap_x8, &bar_full[stage], P.x_start, y0, zin, col);
-            tma_load_4d(dst + 2 * TY * row_bytes, &tmap_x8, &bar_full[stage], P.x_start, yb, zin, col);
+#pragma unroll
+            for (int j = 0; j < TYB; ++j)
+                tma_load_4d(dst + (1 + j) * TB * row_bytes, &tmap_x8, &bar_full[stage], P.x_start, y0 + TB * j, zin, col);
+            tma_load_4d(dst + (1 + TYB) * TB * row_bytes, &tmap_x8, &bar_full[stage], P.x_start, yb, zin, col);
             if (do_xy) tma_load_3d(dst + P.psi_bytes, &tmap_v, &bar_full[stage], 0, y0, z0 - R + s);
             if (do_prev) tma_load_4d(dst + P.psi_bytes + P.tile_bytes, &tmap_p, &bar_full[stage], 0, y0, z0 - 2 * R + s, col);
             if (++stage == P.nstage) { stage = 0; phase ^= 1u; }
@@ -190,10 +195,12 @@ stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
     }
 
     // ==================================== consumer warps ====================================================
-    const int cw = (tid >> 5) - 1;             // 8-wide x block of this warp
+    const int cw = (tid >> 5) - 1;             // (row block, 8-wide x block) of this warp
     if (cw >= P.nwarps) return;
     const int lane = tid & 31, lq = lane & 3, lr = lane >> 2;
-    const int x0 = 8 * cw;
+    const int rb = cw / P.nxb;                  // 8-row block of the tile
+    const int x0 = 8 * (cw - rb * P.nxb);
+    const int ry = TB * rb;
     const int xoff = P.per_x ? 0 : R;           // halo columns are stored only for a Dirichlet x axis
     // Toeplitz fragments: tap distance d = (k - 6) - (output index), k = 4 s + lq; the centre tap is pointwise
     double ay[KS], bx[KS];
@@ -207,14 +214,14 @@ stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
         int xc = x0 - R + 4 * s + lq;
         if (P.per_x) { if (xc < 0) xc += P.nx; else if (xc >= P.nx) xc -= P.nx; }
         else xc += R;
-        xa[s] = (uint32_t)(((TY + lr) * W + xc) * 8);
+        xa[s] = (uint32_t)(((TB + ry + lr) * W + xc) * 8);
     }
-    const uint32_t ya0 = (uint32_t)(((TY - R + lq) * W + x0 + lr + xoff) * 8);      // row y0 - 6 + lq, + s * 4 rows
+    const uint32_t ya0 = (uint32_t)(((TB - R + ry + lq) * W + x0 + lr + xoff) * 8);      // row y0 + ry - 6 + lq, + s * 4 rows
     const uint32_t ystep = (uint32_t)(4 * W * 8);
-    const uint32_t own_off = (uint32_t)(((TY + lr) * W + x0 + 2 * lq + xoff) * 8);
-    const uint32_t tile_off = P.psi_bytes + (uint32_t)((lr * W + x0 + 2 * lq) * 8);
+    const uint32_t own_off = (uint32_t)(((TB + ry + lr) * W + x0 + 2 * lq + xoff) * 8);
+    const uint32_t tile_off = P.psi_bytes + (uint32_t)(((ry + lr) * W + x0 + 2 * lq) * 8);
     const int64_t plane = (int64_t)P.nx * P.ny;
-    double *out_z = P.out + (int64_t)col * P.ldo + (int64_t)(y0 + lr) * P.nx + x0 + 2 * lq + (int64_t)(z0 - 2 * R) * plane;
+    double *out_z = P.out + (int64_t)col * P.ldo + (int64_t)(y0 + ry + lr) * P.nx + x0 + 2 * lq + (int64_t)(z0 - 2 * R) * plane;
 
     double acc[NSLOT][2];
 #pragma unroll
@@ -323,7 +330,7 @@ bool stencil_dmma_supported(const sparc_gpu_ctx *ctx, const double *X, int64_t l
     if (!ctx->fn_encode_tiled || ctx->radius != R) return false;
     const int nx = ctx->n[0], ny = ctx->n[1];
     if (nx % 8 || nx < 16 || nx > 96) return false;          // <= 12 consumer warps
-    if (ny % TY || ny < 2 * TY) return false;
+    if (ny % TB || ny < 2 * TB) return false;
     if (pick_pitch(ctx->bc[0] == 0 ? nx : nx + 2 * R) > 256) return false;
     if (!a16(X) || !a16(Out) || (Prev && !a16(Prev)) || (ldx & 1) || (ldo & 1) || (Prev && (ldp & 1))) return false;
     return true;
@@ -344,16 +351,22 @@ int launch_stencil_dmma(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double
     P.per_x = ctx->bc[0] == 0; P.per_y = ctx->bc[1] == 0; P.per_z = ctx->bc[2] == 0;
     P.W = pick_pitch(P.per_x ? nx : nx + 2 * R);
     P.x_start = P.per_x ? 0 : -R;
-    P.nwarps = nx / 8;
+    // 16-row tiles (a third less halo traffic) when 2 nx / 8 consumer warps still fit the 12-warp kernel
+    const int tyb = (ctx->opt_stencil_ty != 8 && ny % (2 * TB) == 0 && 2 * (nx / 8) <= 12) ? 2 : 1;
+    const int TY = TB * tyb;
+    P.nxb = nx / 8;
+    P.nwarps = tyb * P.nxb;
     P.ytiles = ny / TY;
-    P.psi_bytes = (uint32_t)(3 * TY * P.W * 8);
+    P.psi_bytes = (uint32_t)((tyb + 2) * TB * P.W * 8);
     P.tile_bytes = (uint32_t)(TY * P.W * 8);
     P.stage_bytes = P.psi_bytes + 2 * P.tile_bytes;
     const int threads = (P.nwarps + 1) * 32;
-    auto kern = has_prev ? stencil_dmma_kernel<true> : stencil_dmma_kernel<false>;
-    // ring depth: three stages, more when shared memory is plentiful (one or two CTAs per SM by registers)
+    auto kern = tyb == 2 ? (has_prev ? stencil_dmma_kernel<true, 2> : stencil_dmma_kernel<false, 2>)
+                         : (has_prev ? stencil_dmma_kernel<true, 1> : stencil_dmma_kernel<false, 1>);
+    // ring depth: as deep as shared memory allows (one or two CTAs per SM by registers); the kernel waits on TMA data
+    // more than on anything else
     const int ctas = threads <= 256 ? 2 : 1;
-    int nstage = (int)std::min<int64_t>(ctx->opt_stencil_stages > 0 ? ctx->opt_stencil_stages : 4,
+    int nstage = (int)std::min<int64_t>(ctx->opt_stencil_stages > 0 ? ctx->opt_stencil_stages : (ctas == 1 ? 8 : 6),
                                         (227 * 1024 / ctas - 2048) / P.stage_bytes);
     nstage = std::min(nstage, MAX_STAGES);
     if (nstage < 2) return SPARC_GPU_UNSUPPORTED;
@@ -362,7 +375,7 @@ int launch_stencil_dmma(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double
     SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
 
     CUtensorMap tmap_v;
-    if (!encode_map(ctx, &tmap_v, ctx->d_veff, 3, 1, ctx->nd, P.W, TY)) return SPARC_GPU_CUDA_ERROR;
+    if (!encode_map(ctx, &tmap_v, ctx->d_veff, 3, 1, ctx->nd, P.W, TY)) return SPARC_GPU_CUDA_ERROR;   // whole tile
     const int64_t max_cols_per_launch = std::max<int64_t>(1, (int64_t)INT32_MAX / ((int64_t)P.ytiles * nz));
     for (int64_t j0 = 0; j0 < ncols; j0 += max_cols_per_launch) {
         const int64_t nb = std::min<int64_t>(max_cols_per_launch, ncols - j0);
@@ -375,7 +388,7 @@ int launch_stencil_dmma(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double
         P.zchunks = (nz + P.zchunk_len - 1) / P.zchunk_len;
         P.out = Out + j0 * ldo;
         CUtensorMap tmap_x, tmap_p;
-        if (!encode_map(ctx, &tmap_x, X + j0 * ldx, 4, nb, ldx, P.W, TY)) return SPARC_GPU_CUDA_ERROR;
+        if (!encode_map(ctx, &tmap_x, X + j0 * ldx, 4, nb, ldx, P.W, TB)) return SPARC_GPU_CUDA_ERROR;
         if (!encode_map(ctx, &tmap_p, has_prev ? Prev + j0 * ldp : X + j0 * ldx, 4, nb, has_prev ? ldp : ldx, P.W, TY))
             return SPARC_GPU_CUDA_ERROR;
         const unsigned grid = (unsigned)(nb * P.ytiles * P.zchunks);
