@@ -49,7 +49,7 @@ def measured_peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    """nvidia-smi clocks / throttle reasons sampled every 50 ms during the timed region."""
 
     FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
               "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -63,7 +63,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(
-                ["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits", "-lms", "200",
+                ["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits", "-lms", "50",
                  "-i", str(self.dev)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._pump, daemon=True)
             self.thread.start()
@@ -83,20 +83,21 @@ class ClockSampler:
             self.proc.wait(timeout=2)
         except Exception:
             self.proc.kill()
-        sm, smax, reasons = [], None, set()
+        sm, smax, pmax, reasons = [], None, None, set()
         for ln in self.lines:
             f = [x.strip() for x in ln.split(",")]
             if len(f) < 9:
                 continue
             try:
                 sm.append(float(f[1])); smax = float(f[2])
+                pmax = max(pmax or 0.0, float(f[3]))
             except ValueError:
                 continue
             for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
                 if val.lower().startswith("active"):
                     reasons.add(name)
-        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": smax,
-                "samples": len(sm), "reasons": sorted(reasons)}
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_min_mhz": min(sm) if sm else None,
+                "sm_max_mhz": smax, "power_w_max": pmax, "samples": len(sm), "reasons": sorted(reasons)}
 
 
 def oracle_filter_rate(wl, ncols, acc="f64"):
@@ -303,9 +304,13 @@ def run_ours(args):
                                           "measured now (sparc_gpu_probe_peak, FP64 %s)" % ("DMMA" if nlk == 9 else "DFMA"),
                                           note="algorithmic flop 4*c*P per pt*orb*deg; padding flop of partial octets not counted")
         # GEMMs: 2*Nd*Ns^2 flop per product; project = Hs (by column blocks) + Ms, rotate = Psi Q
-        rooflines["gemm_tn"] = entry("gemm_tn", "tensor", prof_s[4][0], prof_s[4][1], reps * 2 * 2.0 * nd * ns * ns,
-                                     dmma_peak, "TFLOP/s", "measured now (sparc_gpu_probe_peak, FP64 DMMA)")
-        rooflines["gemm_nn"] = entry("gemm_nn", "tensor", prof_s[5][0], prof_s[5][1], reps * 2.0 * nd * ns * ns,
+        # (flop ISSUED, counted by the library: Hs and Ms are computed as upper-triangle tiles + mirror, reading R12,
+        # so the TN kernels issue about half of the nominal 2 x 2*Nd*Ns^2; no credit for skipped work)
+        rooflines["gemm_tn"] = entry("gemm_tn", "tensor", prof_s[4][0], prof_s[4][1], g.get_info("gemm_tn_mflop") * 1e6,
+                                     dmma_peak, "TFLOP/s", "measured now (sparc_gpu_probe_peak, FP64 DMMA)",
+                                     note="flop issued (upper-triangle tiles incl. tile padding); nominal full products: %.3e"
+                                          % (reps * 2 * 2.0 * nd * ns * ns))
+        rooflines["gemm_nn"] = entry("gemm_nn", "tensor", prof_s[5][0], prof_s[5][1], g.get_info("gemm_nn_mflop") * 1e6,
                                      dmma_peak, "TFLOP/s", "measured now (sparc_gpu_probe_peak, FP64 DMMA)")
         rooflines = {k: v for k, v in rooflines.items() if v}
         roofline = dict(max(rooflines.values(), key=lambda e: e["share_of_step"]))
@@ -341,6 +346,9 @@ def run_ours(args):
                        "l2": f"Psi block ({ns * ld * 8 / 1e6:.0f} MB) is larger than the 126 MB L2 and is regenerated between steps"},
             "hbm_gbs": value * ALG_BYTES_PER_UNIT / 1e9,
             "subspace_tflops": sub_flops / ((proj + rot) * 1e-3) / 1e12,
+            "subspace_tflops_note": "nominal 3 x 2*Nd*Ns^2 flop over (project + rotate) time; Hs and Ms are computed as "
+                                    "upper-triangle tiles + mirror, so this is time-to-result, not issued flop "
+                                    "(see roofline_by_kernel for issued flop)",
             "step_ms": {"filter": filt, "project": proj, "rotate": rot, "wall_per_step": t_wall / args.steps * 1e3},
             "clocks": clocks,
             "e2e": {"value": float(nd) * ns_e2e * m * world / e2e_s, "unit": UNIT,
@@ -363,7 +371,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=40)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=1)
     ap.add_argument("--col-block", type=int, default=0)

@@ -399,12 +399,14 @@ int sparc_gpu_set_option(sparc_gpu_ctx *ctx, const char *key, int64_t value)
         if (!ctx->prof) return SPARC_GPU_OUT_OF_MEMORY;
         prof_collect(ctx->prof);
         for (int k = 0; k < KK_COUNT; ++k) { ctx->prof->ns[k] = 0; ctx->prof->count[k] = 0; }
+        ctx->gemm_flop[0] = ctx->gemm_flop[1] = 0.0;
         return 0;
     }
     if (!strcmp(key, "stencil_ay")) { ctx->opt_stencil_ay = (int)value; return 0; }
     if (!strcmp(key, "stencil_ty")) { ctx->opt_stencil_ty = (int)value; return 0; }
     if (!strcmp(key, "stencil_stages")) { ctx->opt_stencil_stages = (int)value; return 0; }
     if (!strcmp(key, "stencil_zchunks")) { ctx->opt_stencil_zchunks = (int)value; return 0; }
+    if (!strcmp(key, "gemm_full")) { ctx->opt_gemm_full = value ? 1 : 0; return 0; }
     if (!strcmp(key, "gemm_path")) { if (value < 0 || value > 2) return SPARC_GPU_INVALID_ARG; ctx->opt_gemm_path = (int)value; return 0; }
     return SPARC_GPU_INVALID_ARG;
 }
@@ -418,6 +420,8 @@ int sparc_gpu_get_info(const sparc_gpu_ctx *ctx, const char *key, int64_t *value
     if (!strcmp(key, "covered_points")) { *value = ctx->n_covered; return 0; }
     if (!strcmp(key, "stencil_path_last")) { *value = ctx->stencil_path_last; return 0; }
     if (!strcmp(key, "sm_count")) { *value = ctx->sm_count; return 0; }
+    if (!strcmp(key, "gemm_tn_mflop")) { *value = (int64_t)(ctx->gemm_flop[0] / 1e6); return 0; }
+    if (!strcmp(key, "gemm_nn_mflop")) { *value = (int64_t)(ctx->gemm_flop[1] / 1e6); return 0; }
     if (!strcmp(key, "nl_brick")) { *value = ctx->nlb.ok; return 0; }
     if (!strcmp(key, "nl_brick_blocks")) { *value = ctx->nlb.n_blocks; return 0; }
     if (!strcmp(key, "nl_brick_active")) { *value = ctx->nlb.n_active; return 0; }
@@ -522,13 +526,19 @@ int sparc_gpu_project(sparc_gpu_ctx *ctx, const double *Psi, int64_t ld, int64_t
     double *Y = (double *)((char *)ws + L.off_w);
     double *D = (double *)((char *)ws + L.off_d);
     void *G = (char *)ws + L.off_g;
+    // Hs and Ms are symmetric (H is): only tiles at or above the diagonal are computed, then mirrored (reading R12)
+    const bool sym = ctx->opt_gemm_full == 0;
     for (int64_t j0 = 0; j0 < ns; j0 += L.block) {
         const int64_t nb = std::min(L.block, ns - j0);
         SPARC_TRY(h_apply_block(ctx, Psi + j0 * ld, ld, Y, L.ldw, nb, D, st));
         // Hs[:, j0:j0+nb] = Psi^T Y_block
-        SPARC_TRY(launch_gemm_tn(ctx, Psi, ld, Y, L.ldw, Hs + j0 * ns, ns, ns, nb, ctx->nd, G, st));
+        SPARC_TRY(launch_gemm_tn(ctx, Psi, ld, Y, L.ldw, Hs + j0 * ns, ns, ns, nb, ctx->nd, G, sym ? j0 : -1, st));
     }
-    SPARC_TRY(launch_gemm_tn(ctx, Psi, ld, Psi, ld, Ms, ns, ns, ns, ctx->nd, G, st));
+    SPARC_TRY(launch_gemm_tn(ctx, Psi, ld, Psi, ld, Ms, ns, ns, ns, ctx->nd, G, sym ? 0 : -1, st));
+    if (sym) {
+        SPARC_TRY(launch_mirror_upper(ctx, Hs, ns, ns, st));
+        SPARC_TRY(launch_mirror_upper(ctx, Ms, ns, ns, st));
+    }
     return SPARC_GPU_SUCCESS;
 }
 

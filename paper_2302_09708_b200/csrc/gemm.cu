@@ -78,7 +78,7 @@ __device__ __forceinline__ void load_tile(double *s, const double *g, int64_t ld
 template <bool A_MMAJOR, bool VEC16, int NWN>
 __global__ void __launch_bounds__(64 * NWN, NWN == 2 ? 2 : 1)
 gemm_dmma_kernel(const double *__restrict__ A, int64_t lda, const double *__restrict__ B, int64_t ldb, double *C,
-                 int64_t ldc, int64_t M, int64_t N, int64_t K, int64_t k_chunk, int tiles_m)
+                 int64_t ldc, int64_t M, int64_t N, int64_t K, int64_t k_chunk, int tiles_m, int64_t diag)
 {
     extern __shared__ __align__(16) double smem[];
     constexpr int BN = 32 * NWN, GEMM_THREADS = 64 * NWN;
@@ -91,6 +91,9 @@ gemm_dmma_kernel(const double *__restrict__ A, int64_t lda, const double *__rest
     const int wm = warp / NWN, wn = warp % NWN;       // 2 x NWN warps, warp tile 64 x 32
     const int tile_m = blockIdx.x % tiles_m, tile_n = blockIdx.x / tiles_m;
     const int64_t m0 = (int64_t)tile_m * BM, n0 = (int64_t)tile_n * BN;
+    // symmetric result (diag >= 0: global column index of column 0): tiles strictly below the diagonal are skipped,
+    // the caller mirrors the upper triangle afterwards
+    if (diag >= 0 && m0 >= diag + n0 + BN) return;
     const int64_t k_begin = (int64_t)blockIdx.z * k_chunk;
     const int64_t k_end = (k_begin + k_chunk < K) ? k_begin + k_chunk : K;
     if (gridDim.z > 1) { C += (int64_t)blockIdx.z * M * N; ldc = M; }
@@ -182,18 +185,49 @@ gemm_simple_kernel(const double *__restrict__ A, int64_t lda, const double *__re
     C[m + n * ldc] = s;
 }
 
+// C[i, j] = C[j, i] for i > j (n x n, column-major): 32 x 32 tiles through shared memory, both sides coalesced
+__global__ void __launch_bounds__(256)
+mirror_upper_kernel(double *C, int64_t ldc, int64_t n)
+{
+    __shared__ double t[32][33];
+    const int64_t bi = blockIdx.x, bj = blockIdx.y;          // destination tile (rows bi, columns bj), bi >= bj
+    if (bi < bj) return;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    for (int r = ty; r < 32; r += 8) {                        // source tile: rows bj*32.., columns bi*32..
+        const int64_t row = bj * 32 + tx, col = bi * 32 + r;
+        t[r][tx] = (row < n && col < n) ? C[row + col * ldc] : 0.0;
+    }
+    __syncthreads();
+    for (int r = ty; r < 32; r += 8) {
+        const int64_t row = bi * 32 + tx, col = bj * 32 + r;  // destination element (row, col) = source (col, row)
+        if (row < n && col < n && row > col) C[row + col * ldc] = t[tx][r];
+    }
+}
+
 struct SplitPlan { int splits; int64_t k_chunk; };
 
 // Split-K plan for the tall contraction (K = N_d >> M, N): the number of CTAs (tiles x splits) is chosen as the
 // nearest-to-whole number of waves over the SMs (one CTA per SM), preferring few splits; partial products go to the
 // workspace and are summed in a fixed order (deterministic).
-SplitPlan plan_tn(const sparc_gpu_ctx *ctx, int64_t M, int64_t N, int64_t K)
+// number of 128 x 64 tiles a launch computes (all, or those at / above the diagonal of a symmetric result)
+int64_t tiles_computed(int64_t M, int64_t N, int64_t diag)
 {
     const int BN = 32 * NWN_DEFAULT;
-    const int64_t tiles = ((M + BM - 1) / BM) * ((N + BN - 1) / BN);
+    const int64_t tm = (M + BM - 1) / BM, tn = (N + BN - 1) / BN;
+    if (diag < 0) return tm * tn;
+    int64_t c = 0;
+    for (int64_t n = 0; n < tn; ++n) c += std::min<int64_t>(tm, (diag + n * BN + BN + BM - 1) / BM);   // tiles with m0 < diag + n0 + BN
+    return c;
+}
+
+int64_t splitk_ws_cap(int64_t M, int64_t N) { return std::min<int64_t>((int64_t)2 << 30, 64 * M * N * 8); }
+
+SplitPlan plan_tn(const sparc_gpu_ctx *ctx, int64_t M, int64_t N, int64_t K, int64_t diag)
+{
+    const int64_t tiles = std::max<int64_t>(1, tiles_computed(M, N, diag));
     const int64_t sms = std::max(1, ctx->sm_count) * (NWN_DEFAULT == 2 ? 2 : 1);      // CTA slots
     const int64_t max_splits = std::max<int64_t>(1, std::min<int64_t>(64, K / (16 * BK)));
-    const int64_t ws_cap = (int64_t)2 << 30;                       // at most 2 GiB of partial products
+    const int64_t ws_cap = splitk_ws_cap(M, N);                   // at most 2 GiB of partial products
     int64_t best_s = 1;
     double best_cost = 1e300;
     for (int64_t s = 1; s <= max_splits; ++s) {
@@ -215,7 +249,7 @@ bool aligned16(const void *p) { return ((uintptr_t)p & 15) == 0; }
 
 template <bool A_MMAJOR>
 int launch_dmma(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const double *B, int64_t ldb, double *C, int64_t ldc,
-                int64_t M, int64_t N, int64_t K, SplitPlan plan, cudaStream_t st)
+                int64_t M, int64_t N, int64_t K, SplitPlan plan, int64_t diag, cudaStream_t st)
 {
     constexpr int NWN = NWN_DEFAULT, BN = 32 * NWN, GEMM_THREADS = 64 * NWN;
     const int tiles_m = (int)((M + BM - 1) / BM), tiles_n = (int)((N + BN - 1) / BN);
@@ -223,16 +257,20 @@ int launch_dmma(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const double *
     const bool vec = aligned16(A) && aligned16(B) && (lda % 2 == 0) && (ldb % 2 == 0);
     const size_t smem = smem_bytes(A_MMAJOR, NWN);
     const int kind = A_MMAJOR ? KK_GEMM_NN : KK_GEMM_TN;
+    {   // flop actually issued (tiles below the diagonal of a symmetric result are skipped; edge tiles count in full)
+        const int64_t computed = tiles_computed(M, N, diag);
+        ctx->gemm_flop[A_MMAJOR ? 1 : 0] += 2.0 * (double)K * (double)(BM * BN) * (double)computed;
+    }
     if (vec) {
         auto kern = gemm_dmma_kernel<A_MMAJOR, true, NWN>;
         SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         prof_begin(ctx, kind, st);
-        kern<<<grid, GEMM_THREADS, smem, st>>>(A, lda, B, ldb, C, ldc, M, N, K, plan.k_chunk, tiles_m);
+        kern<<<grid, GEMM_THREADS, smem, st>>>(A, lda, B, ldb, C, ldc, M, N, K, plan.k_chunk, tiles_m, diag);
     } else {
         auto kern = gemm_dmma_kernel<A_MMAJOR, false, NWN>;
         SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         prof_begin(ctx, kind, st);
-        kern<<<grid, GEMM_THREADS, smem, st>>>(A, lda, B, ldb, C, ldc, M, N, K, plan.k_chunk, tiles_m);
+        kern<<<grid, GEMM_THREADS, smem, st>>>(A, lda, B, ldb, C, ldc, M, N, K, plan.k_chunk, tiles_m, diag);
     }
     prof_end(ctx, kind, st);
     SPARC_CUDA_TRY(cudaGetLastError());
@@ -243,12 +281,12 @@ int launch_dmma(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const double *
 
 int64_t gemm_tn_ws_bytes(const sparc_gpu_ctx *ctx, int64_t M, int64_t N, int64_t K)
 {
-    SplitPlan p = plan_tn(ctx, M, N, K);
-    return p.splits > 1 ? (int64_t)p.splits * M * N * 8 : 0;
+    (void)ctx; (void)K;
+    return splitk_ws_cap(M, N);        // upper bound of any split-K plan (the plan depends on the tiles actually computed)
 }
 
 int launch_gemm_tn(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const double *B, int64_t ldb, double *C,
-                   int64_t ldc, int64_t M, int64_t N, int64_t K, void *ws, cudaStream_t st)
+                   int64_t ldc, int64_t M, int64_t N, int64_t K, void *ws, int64_t diag, cudaStream_t st)
 {
     if (M <= 0 || N <= 0) return SPARC_GPU_SUCCESS;
     if (ctx->opt_gemm_path == 1) {
@@ -259,10 +297,10 @@ int launch_gemm_tn(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const doubl
         SPARC_CUDA_TRY(cudaGetLastError());
         return SPARC_GPU_SUCCESS;
     }
-    SplitPlan plan = plan_tn(ctx, M, N, K);
+    SplitPlan plan = plan_tn(ctx, M, N, K, diag);
     if (plan.splits > 1) {
         double *part = (double *)ws;
-        SPARC_TRY(launch_dmma<false>(ctx, A, lda, B, ldb, part, M, M, N, K, plan, st));
+        SPARC_TRY(launch_dmma<false>(ctx, A, lda, B, ldb, part, M, M, N, K, plan, diag, st));     // skipped tiles stay undefined
         int64_t blocks = std::min<int64_t>((M * N + 255) / 256, (int64_t)ctx->sm_count * 8);
         prof_begin(ctx, KK_SPLITK_REDUCE, st);
         splitk_reduce_kernel<<<(unsigned)blocks, 256, 0, st>>>(part, plan.splits, M, N, C, ldc);
@@ -270,7 +308,7 @@ int launch_gemm_tn(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const doubl
         SPARC_CUDA_TRY(cudaGetLastError());
         return SPARC_GPU_SUCCESS;
     }
-    return launch_dmma<false>(ctx, A, lda, B, ldb, C, ldc, M, N, K, plan, st);
+    return launch_dmma<false>(ctx, A, lda, B, ldb, C, ldc, M, N, K, plan, diag, st);
 }
 
 int launch_gemm_nn(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const double *B, int64_t ldb, double *C,
@@ -286,5 +324,16 @@ int launch_gemm_nn(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const doubl
         return SPARC_GPU_SUCCESS;
     }
     SplitPlan plan{1, round_up_i64(std::max<int64_t>(K, 1), BK)};
-    return launch_dmma<true>(ctx, A, lda, B, ldb, C, ldc, M, N, K, plan, st);
+    return launch_dmma<true>(ctx, A, lda, B, ldb, C, ldc, M, N, K, plan, -1, st);
+}
+
+int launch_mirror_upper(sparc_gpu_ctx *ctx, double *C, int64_t ldc, int64_t n, cudaStream_t st)
+{
+    if (n <= 1) return SPARC_GPU_SUCCESS;
+    const unsigned nt = (unsigned)((n + 31) / 32);
+    prof_begin(ctx, KK_COPY2D, st);
+    mirror_upper_kernel<<<dim3(nt, nt), 256, 0, st>>>(C, ldc, n);
+    prof_end(ctx, KK_COPY2D, st);
+    SPARC_CUDA_TRY(cudaGetLastError());
+    return SPARC_GPU_SUCCESS;
 }

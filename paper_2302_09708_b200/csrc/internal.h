@@ -73,6 +73,7 @@ struct sparc_gpu_ctx {
     int opt_stencil_path;      // 0 auto, 1 generic, 2 TMA (DFMA), 3 TMA + DMMA in-plane taps
     int opt_nonlocal;          // 1 on
     int opt_gemm_path;         // 0 auto, 1 simple, 2 DMMA
+    int opt_gemm_full;         // 0: Hs, Ms computed as upper triangle + mirror (R12); 1: all tiles
     int opt_nonlocal_mode;     // 0 auto (brick kernel when supported, else 2), 1 project + pull (deterministic),
                                // 2 fused per-atom kernel with atomic scatter, 3 brick kernel or UNSUPPORTED
     int opt_stencil_ay;        // 0 auto, 1 or 2: rows per consumer thread of the TMA stencil kernel
@@ -81,6 +82,7 @@ struct sparc_gpu_ctx {
     int opt_stencil_zchunks;   // 0 auto, else forced number of z chunks
     // counters
     mutable int64_t kernel_launches;
+    double gemm_flop[2];       // flop issued by the DMMA GEMMs since the last "profile_reset": [0] TN, [1] NN
     int stencil_path_last;
     // driver entry point for tensor-map encoding (resolved at create; NULL if unavailable)
     void *fn_encode_tiled;
@@ -158,10 +160,13 @@ int launch_nl_brick(sparc_gpu_ctx *ctx, int mode, double *XorOut, int64_t ld, in
                     const double *c_in, double *c_out, cudaStream_t st);
 
 // C (M x N, col-major, ldc) = A^T B, A: K x M (lda), B: K x N (ldb), contraction over K rows.
-// ws: split-K partials (gemm_tn_ws_bytes).  symmetric_out: A == B, fill lower from upper.
+// ws: split-K partials (gemm_tn_ws_bytes).  diag >= 0: the result is (a column block, starting at global column diag,
+// of) a symmetric matrix: tiles strictly below the diagonal may be skipped (launch_mirror_upper fills them in).
 int64_t gemm_tn_ws_bytes(const sparc_gpu_ctx *ctx, int64_t M, int64_t N, int64_t K);
 int launch_gemm_tn(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const double *B, int64_t ldb,
-                   double *C, int64_t ldc, int64_t M, int64_t N, int64_t K, void *ws, cudaStream_t st);
+                   double *C, int64_t ldc, int64_t M, int64_t N, int64_t K, void *ws, int64_t diag, cudaStream_t st);
+// C[i, j] = C[j, i] for i > j (after a launch_gemm_tn with diag >= 0)
+int launch_mirror_upper(sparc_gpu_ctx *ctx, double *C, int64_t ldc, int64_t n, cudaStream_t st);
 // C (M x N, ldc) = A B, A: M x K col-major (lda), B: K x N col-major (ldb)
 int launch_gemm_nn(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const double *B, int64_t ldb,
                    double *C, int64_t ldc, int64_t M, int64_t N, int64_t K, cudaStream_t st);

@@ -293,6 +293,25 @@ def test_config1_full(torch, api):
     full_config_parity(torch, api, 1)
 
 
+def test_project_symmetric_tiles_and_mirror(torch, api):
+    """Hs and Ms computed as upper-triangle tiles + mirror (reading R12; the path configs 3-4 take) against the oracle's
+    full sums and against the all-tiles path, on a shape with several 128 x 64 tiles and ragged edges."""
+    wl = wlmod.make_custom("symtiles", (6, 6, 6), (0.5,) * 3, (1, 1, 1), 200, 2, np.array([[1.2, 1.4, 1.1]]), [4], 1.2)
+    g = api.SparcGpu(wl)
+    X = wl.psi_columns(range(wl.ns))
+    Hs_o, Ms_o = orc.Hamiltonian(wl).project(X)
+    out = {}
+    for full in (0, 1):
+        g.set_option("gemm_full", full)
+        Hs, Ms = g.project(api.colmajor_from_numpy(X), col_block=70)
+        out[full] = (api.colmajor_to_numpy(Hs), api.colmajor_to_numpy(Ms))
+        check_fro(out[full][0], Hs_o, f"Hs gemm_full={full}")
+        check_fro(out[full][1], Ms_o, f"Ms gemm_full={full}")
+    assert np.array_equal(out[0][0], out[0][0].T) and np.array_equal(out[0][1], out[0][1].T)     # mirrored exactly
+    assert np.array_equal(np.triu(out[0][1]), np.triu(out[1][1]))                                # same upper triangle
+    g.close()
+
+
 def test_gemm_paths_agree_and_ragged_shapes(torch, api):
     """DMMA GEMMs on shapes that are not multiples of the tile, odd leading dimensions (8-byte copy path)."""
     wl = wlmod.make_custom("rag", (15, 14, 13), (0.5,) * 3, (1, 1, 1), 37, 2, np.array([[3.0, 3.0, 3.0]]), [4], 2.0)
