@@ -163,6 +163,10 @@ def run_ours(args):
 
     wl = wlmod.make_workload(args.config)
     g = api.SparcGpu(wl, device=local_rank)
+    if args.stencil_path:
+        g.set_option("stencil_path", args.stencil_path)
+    if args.stencil_stages:
+        g.set_option("stencil_stages", args.stencil_stages)
     nd, ns, m = wl.nd, wl.ns, wl.degree
     ld = nd
     psi = torch.empty((ns, ld), dtype=torch.float64, device=dev)
@@ -342,7 +346,7 @@ def run_ours(args):
             "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": wl.name, "grid": list(wl.n), "nd": nd, "ns": ns, "degree": m,
-                       "atoms": wl.n_atoms, "col_block": col_block, "parallelism": f"replicas x{world}",
+                       "atoms": wl.n_atoms, "col_block": col_block, "stencil_path": g.get_info("stencil_path_last"), "parallelism": f"replicas x{world}",
                        "l2": f"Psi block ({ns * ld * 8 / 1e6:.0f} MB) is larger than the 126 MB L2 and is regenerated between steps"},
             "hbm_gbs": value * ALG_BYTES_PER_UNIT / 1e9,
             "subspace_tflops": sub_flops / ((proj + rot) * 1e-3) / 1e12,
@@ -377,6 +381,8 @@ def main():
     ap.add_argument("--col-block", type=int, default=0)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
+    ap.add_argument("--stencil-path", type=int, default=0, help="0 library default, 2 TMA + DFMA kernel, 3 TMA + DMMA hybrid")
+    ap.add_argument("--stencil-stages", type=int, default=0, help="TMA ring depth (0 = library default)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

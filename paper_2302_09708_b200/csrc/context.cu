@@ -189,7 +189,11 @@ int local_pass(sparc_gpu_ctx *c, const double *X, int64_t ldx, double *Out, int6
                int64_t ldp, int64_t ncols, double alpha, double shift, double beta, cudaStream_t st)
 {
     int path = c->opt_stencil_path;
-    if (path == 0) path = stencil_tma_supported(c, X, ldx, Out, ldo, Prev, ldp) ? 2 : 1;
+    if (path == 0) {
+        // wide grids (12 x-blocks): the hybrid DMMA kernel is ~5 % ahead (configs 3-4); otherwise the DFMA kernel
+        if (c->n[0] >= 64 && stencil_dmma_supported(c, X, ldx, Out, ldo, Prev, ldp)) path = 3;
+        else path = stencil_tma_supported(c, X, ldx, Out, ldo, Prev, ldp) ? 2 : 1;
+    }
     if (path == 3) {
         SPARC_TRY(launch_stencil_dmma(c, X, ldx, Out, ldo, Prev, ldp, ncols, alpha, shift, beta, st));
     } else if (path == 2) {

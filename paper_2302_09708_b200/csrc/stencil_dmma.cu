@@ -366,7 +366,7 @@ int launch_stencil_dmma(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double
     // ring depth: as deep as shared memory allows (one or two CTAs per SM by registers); the kernel waits on TMA data
     // more than on anything else
     const int ctas = threads <= 256 ? 2 : 1;
-    int nstage = (int)std::min<int64_t>(ctx->opt_stencil_stages > 0 ? ctx->opt_stencil_stages : (ctas == 1 ? 8 : 6),
+    int nstage = (int)std::min<int64_t>(ctx->opt_stencil_stages > 0 ? ctx->opt_stencil_stages : 6,
                                         (227 * 1024 / ctas - 2048) / P.stage_bytes);
     nstage = std::min(nstage, MAX_STAGES);
     if (nstage < 2) return SPARC_GPU_UNSUPPORTED;
