@@ -31,6 +31,7 @@ constexpr int MAX_STAGES = 8;
 struct DmParams {
     double cx[R + 1], cy[R + 1], cz[R + 1];   // alpha * (-1/2 w_p / h^2)
     double c0a;                                // alpha * (c0 + shift)
+    double rxy;                                // cx[p] / cy[p] = (h_y / h_x)^2: one Toeplitz fragment set serves both axes
     double alpha, beta;
     double *out;
     int64_t ldo;
@@ -123,8 +124,8 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
                  : "d"(a), "d"(b));
 }
 
-template <bool HAS_PREV, int TYB>
-__global__ void __launch_bounds__(13 * 32, 1)
+template <bool HAS_PREV, int TYB, int MINB>
+__global__ void __launch_bounds__(MINB == 1 ? 13 * 32 : 7 * 32, MINB)
 stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
                     const __grid_constant__ CUtensorMap tmap_v, const __grid_constant__ CUtensorMap tmap_p,
                     const __grid_constant__ DmParams P)
@@ -203,14 +204,13 @@ stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
     const int ry = TB * rb;
     const int xoff = P.per_x ? 0 : R;           // halo columns are stored only for a Dirichlet x axis
     // Toeplitz fragments: tap distance d = (k - 6) - (output index), k = 4 s + lq; the centre tap is pointwise
-    double ay[KS], bx[KS];
+    double ay[KS];                              // (the x fragments are rxy times the same numbers)
     uint32_t xa[KS];                            // byte offsets of the x-tap data fragments (row y0 + lr, wrapped column)
 #pragma unroll
     for (int s = 0; s < KS; ++s) {
         const int d = 4 * s + lq - R - lr;
         const int ad = d < 0 ? -d : d;
         ay[s] = (ad >= 1 && ad <= R) ? P.cy[ad] : 0.0;
-        bx[s] = (ad >= 1 && ad <= R) ? P.cx[ad] : 0.0;
         int xc = x0 - R + 4 * s + lq;
         if (P.per_x) { if (xc < 0) xc += P.nx; else if (xc >= P.nx) xc -= P.nx; }
         else xc += R;
@@ -253,10 +253,10 @@ stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
 #pragma unroll
                 for (int k = 0; k < KS; ++k) {
                     dmma884(c0, c1, ay[k], fy[k]);        // y taps: constants x data
-                    dmma884(e0, e1, fx[k], bx[k]);        // x taps: data x constants (second chain)
+                    dmma884(e0, e1, fx[k], ay[k]);        // x taps: data x constants (second chain), scaled below
                 }
-                acc[ph][0] = c0 + fma(fma(P.alpha, vf.x, P.c0a), own.x, e0);
-                acc[ph][1] = c1 + fma(fma(P.alpha, vf.y, P.c0a), own.y, e1);
+                acc[ph][0] = c0 + fma(P.rxy, e0, fma(P.alpha, vf.x, P.c0a) * own.x);
+                acc[ph][1] = c1 + fma(P.rxy, e1, fma(P.alpha, vf.y, P.c0a) * own.y);
             }
             // ---- z taps: this plane feeds the 12 neighbouring output planes --------------------------------------
 #pragma unroll
@@ -345,6 +345,7 @@ int launch_stencil_dmma(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double
     DmParams P;
     for (int p = 0; p <= R; ++p) { P.cx[p] = alpha * ctx->coef.cx[p]; P.cy[p] = alpha * ctx->coef.cy[p]; P.cz[p] = alpha * ctx->coef.cz[p]; }
     P.c0a = alpha * (ctx->coef.c0 + shift);
+    P.rxy = (ctx->h[1] * ctx->h[1]) / (ctx->h[0] * ctx->h[0]);
     P.alpha = alpha; P.beta = beta;
     P.ldo = ldo;
     P.nx = nx; P.ny = ny; P.nz = nz;
@@ -352,7 +353,7 @@ int launch_stencil_dmma(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double
     P.W = pick_pitch(P.per_x ? nx : nx + 2 * R);
     P.x_start = P.per_x ? 0 : -R;
     // 16-row tiles (a third less halo traffic) when 2 nx / 8 consumer warps still fit the 12-warp kernel
-    const int tyb = (ctx->opt_stencil_ty != 8 && ny % (2 * TB) == 0 && 2 * (nx / 8) <= 12) ? 2 : 1;
+    const int tyb = (ctx->opt_stencil_ty == 16 && ny % (2 * TB) == 0 && 2 * (nx / 8) <= 12) ? 2 : 1;
     const int TY = TB * tyb;
     P.nxb = nx / 8;
     P.nwarps = tyb * P.nxb;
@@ -361,11 +362,16 @@ int launch_stencil_dmma(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double
     P.tile_bytes = (uint32_t)(TY * P.W * 8);
     P.stage_bytes = P.psi_bytes + 2 * P.tile_bytes;
     const int threads = (P.nwarps + 1) * 32;
-    auto kern = tyb == 2 ? (has_prev ? stencil_dmma_kernel<true, 2> : stencil_dmma_kernel<false, 2>)
-                         : (has_prev ? stencil_dmma_kernel<true, 1> : stencil_dmma_kernel<false, 1>);
+    // up to 6 consumer warps: two CTAs per SM (128 registers; a third would need <= 80 and spills the z-sums);
+    // more: one CTA of up to 12 consumer warps
+    const bool small = P.nwarps <= 6;
+    typedef void (*Kern)(const CUtensorMap, const CUtensorMap, const CUtensorMap, const DmParams);
+    Kern kern = small ? (has_prev ? (Kern)stencil_dmma_kernel<true, 1, 2> : (Kern)stencil_dmma_kernel<false, 1, 2>)
+                : tyb == 2 ? (has_prev ? (Kern)stencil_dmma_kernel<true, 2, 1> : (Kern)stencil_dmma_kernel<false, 2, 1>)
+                           : (has_prev ? (Kern)stencil_dmma_kernel<true, 1, 1> : (Kern)stencil_dmma_kernel<false, 1, 1>);
     // ring depth: as deep as shared memory allows (one or two CTAs per SM by registers); the kernel waits on TMA data
     // more than on anything else
-    const int ctas = threads <= 256 ? 2 : 1;
+    const int ctas = (P.nwarps <= 6 && tyb == 1) ? 2 : 1;
     int nstage = (int)std::min<int64_t>(ctx->opt_stencil_stages > 0 ? ctx->opt_stencil_stages : 6,
                                         (227 * 1024 / ctas - 2048) / P.stage_bytes);
     nstage = std::min(nstage, MAX_STAGES);
