@@ -207,12 +207,16 @@ nl_brick_kernel(const BrickParams p)
     const int32_t *pt_h = pt_off + 2 * lq;
     const double *srcc = p.src + (int64_t)(colv ? col : 0) * p.ld;
     double2 c[NB_HOCT];
+    {
+        // all offsets first, then branch-free loads: an untouched octet reads the column's first pair (a cached dummy)
+        int off[NB_HOCT];
 #pragma unroll
-    for (int o = 0; o < NB_HOCT; ++o) {
-        c[o] = make_double2(0.0, 0.0);
-        if (umask_h & (1u << o)) {
-            const int off = pt_h[8 * o];
-            if (off >= 0 && colv) c[o] = *reinterpret_cast<const double2 *>(srcc + off);
+        for (int o = 0; o < NB_HOCT; ++o) off[o] = pt_h[8 * o];
+#pragma unroll
+        for (int o = 0; o < NB_HOCT; ++o) {
+            const bool ok = ((umask_h >> o) & 1u) && off[o] >= 0 && colv;
+            const double2 v = *reinterpret_cast<const double2 *>(srcc + (ok ? off[o] : 0));
+            c[o] = ok ? v : make_double2(0.0, 0.0);
         }
     }
 
@@ -267,12 +271,13 @@ nl_brick_kernel(const BrickParams p)
             if (lane == 0) mbar_arrive(&empty[slot]);
             if (jj == na - 1) {                            // all atoms pulled: the tile is the final Out
                 double *dstc = p.dst + (int64_t)(colv ? col : 0) * p.ld;
+                int off[NB_HOCT];
+#pragma unroll
+                for (int o = 0; o < NB_HOCT; ++o) off[o] = pt_h[8 * o];
 #pragma unroll
                 for (int o = 0; o < NB_HOCT; ++o) {
-                    if (umask_h & (1u << o)) {
-                        const int off = pt_h[8 * o];
-                        if (off >= 0 && colv) *reinterpret_cast<double2 *>(dstc + off) = c[o];
-                    }
+                    const bool ok = ((umask_h >> o) & 1u) && off[o] >= 0 && colv;
+                    if (ok) *reinterpret_cast<double2 *>(dstc + off[o]) = c[o];
                 }
             }
         } else {
