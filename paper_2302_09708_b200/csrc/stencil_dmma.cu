@@ -38,8 +38,8 @@ struct DmParams {
     int nx, ny, nz;
     int W;            // smem row pitch in doubles (all three tiles)
     int x_start;      // first x coordinate of the boxes: 0 (periodic x) or -6 (Dirichlet x)
-    int nwarps;       // consumer warps = TYB * nx / 8
-    int nxb;          // x blocks = nx / 8
+    int nwarps;       // consumer warps = TYB * nxb
+    int nxb;          // x blocks = ceil(nx / 8): the last one may overhang the grid (its extra columns are not stored)
     int nstage;
     int ytiles, zchunks, zchunk_len;
     int per_x, per_y, per_z;
@@ -202,6 +202,7 @@ stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
     const int rb = cw / P.nxb;                  // 8-row block of the tile
     const int x0 = 8 * (cw - rb * P.nxb);
     const int ry = TB * rb;
+    const bool xvalid = x0 + 2 * (lane & 3) < P.nx;       // n_x is even: a lane's pair is inside or outside as a whole
     const int xoff = P.per_x ? 0 : R;           // halo columns are stored only for a Dirichlet x axis
     // Toeplitz fragments: tap distance d = (k - 6) - (output index), k = 4 s + lq; the centre tap is pointwise
     double ay[KS];                              // (the x fragments are rxy times the same numbers)
@@ -284,7 +285,7 @@ stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
                 double2 o;
                 o.x = HAS_PREV ? fma(P.beta, pv.x, acc[cs][0]) : acc[cs][0];
                 o.y = HAS_PREV ? fma(P.beta, pv.y, acc[cs][1]) : acc[cs][1];
-                *reinterpret_cast<double2 *>(out_z) = o;
+                if (xvalid) *reinterpret_cast<double2 *>(out_z) = o;
             }
             out_z += plane;
             ++s;
@@ -329,9 +330,9 @@ bool stencil_dmma_supported(const sparc_gpu_ctx *ctx, const double *X, int64_t l
 {
     if (!ctx->fn_encode_tiled || ctx->radius != R) return false;
     const int nx = ctx->n[0], ny = ctx->n[1];
-    if (nx % 8 || nx < 16 || nx > 96) return false;          // <= 12 consumer warps
+    if (nx % 2 || nx < 16 || nx > 96) return false;          // <= 12 consumer warps
     if (ny % TB || ny < 2 * TB) return false;
-    if (pick_pitch(ctx->bc[0] == 0 ? nx : nx + 2 * R) > 256) return false;
+    if (pick_pitch((nx + 7) / 8 * 8 + (ctx->bc[0] == 0 ? 0 : 2 * R)) > 256) return false;
     if (!a16(X) || !a16(Out) || (Prev && !a16(Prev)) || (ldx & 1) || (ldo & 1) || (Prev && (ldp & 1))) return false;
     return true;
 }
@@ -350,12 +351,13 @@ int launch_stencil_dmma(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double
     P.ldo = ldo;
     P.nx = nx; P.ny = ny; P.nz = nz;
     P.per_x = ctx->bc[0] == 0; P.per_y = ctx->bc[1] == 0; P.per_z = ctx->bc[2] == 0;
-    P.W = pick_pitch(P.per_x ? nx : nx + 2 * R);
+    P.W = pick_pitch(8 * ((nx + 7) / 8) + (P.per_x ? 0 : 2 * R));
     P.x_start = P.per_x ? 0 : -R;
     // 16-row tiles (a third less halo traffic) when 2 nx / 8 consumer warps still fit the 12-warp kernel
-    const int tyb = (ctx->opt_stencil_ty == 16 && ny % (2 * TB) == 0 && 2 * (nx / 8) <= 12) ? 2 : 1;
+    const int nxb = (nx + 7) / 8;
+    const int tyb = (ctx->opt_stencil_ty == 16 && ny % (2 * TB) == 0 && 2 * nxb <= 12) ? 2 : 1;
     const int TY = TB * tyb;
-    P.nxb = nx / 8;
+    P.nxb = nxb;
     P.nwarps = tyb * P.nxb;
     P.ytiles = ny / TY;
     P.psi_bytes = (uint32_t)((tyb + 2) * TB * P.W * 8);
