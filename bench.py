@@ -136,7 +136,7 @@ def run_reference(args):
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": wl.name, "nd": wl.nd, "ns": wl.ns, "degree": wl.degree, "sample_columns": ncols},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores,
-                         "kind": "oracle (oracle/chefsi_oracle.c, acc_t=double build)", "sample": sample},
+                         "kind": "oracle", "detail": "oracle/chefsi_oracle.c, acc_t = double build, OpenMP over columns", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -333,7 +333,7 @@ def run_ours(args):
             ncols *= 2
             rate, dt = oracle_filter_rate(wl, ncols)
         cpu_baseline = {"value": rate, "unit": UNIT, "cores": cores,
-                        "kind": "oracle (oracle/chefsi_oracle.c, acc_t=double build)",
+                        "kind": "oracle", "detail": "oracle/chefsi_oracle.c, acc_t = double build, OpenMP over columns",
                         "sample": f"Chebyshev filter degree {m} on {ncols} of {ns} columns of {wl.name}: {dt:.1f} s",
                         }
 
