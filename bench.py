@@ -35,8 +35,9 @@ UNIT = "grid-pt*orbital*degree/s"
 ALG_BYTES_PER_UNIT = 24.0       # read Psi_k, read Psi_{k-1}, write Psi_{k+1}
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` capture (profiles/r01b_ncu_stencil_tma_cfg1.md), keyed by (config, kernel).
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {(1, "stencil"): 697.6e6}
+# `ncu --set full` captures, keyed by (config, kernel).
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {(1, "stencil"): 697.6e6,       # profiles/r01b_ncu_kernels_cfg1.md
+                                (3, "stencil"): 23.32e9}       # profiles/r01c_ncu_kernels_cfg3.md (hybrid kernel)
 
 
 def measured_peaks():
