@@ -139,8 +139,9 @@ int sparc_gpu_probe_peak(int device, int kind, double *value_out, void *scratch_
  * "nonlocal" (1 on, 0 off: drops V_nl, used by closed-form pins), "nonlocal_mode" (0 auto = brick-tiled DMMA kernel
  * when supported, 1 project + pull: bitwise reproducible, 2 per-atom fused kernel with atomic scatter, 3 brick kernel
  * or UNSUPPORTED), "gemm_path" (0 auto, 1 simple FMA kernel, 2 DMMA kernel), "profile" / "profile_reset" (per-kernel
- * CUDA-event timing read back through sparc_gpu_get_info "prof_ns:<kind>" / "prof_count:<kind>"), and the stencil
- * tile knobs "stencil_ay", "stencil_ty", "stencil_stages", "stencil_zchunks" (0 = library chooses).
+ * CUDA-event timing read back through sparc_gpu_get_info "prof_ns:<kind>" / "prof_count:<kind>"), "nlb_tma" (0: the brick
+ * kernel stages its tile with TMA, 1: direct global loads / stores), "gemm_full" (0: Hs, Ms as upper-triangle tiles +
+ * mirror, 1: all tiles), and the stencil tile knobs "stencil_ay", "stencil_ty", "stencil_stages", "stencil_zchunks" (0 = library chooses).
  * Unknown key -> INVALID_ARG. */
 int sparc_gpu_set_option(sparc_gpu_ctx *ctx, const char *key, int64_t value);
 

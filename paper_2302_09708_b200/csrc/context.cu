@@ -410,6 +410,7 @@ int sparc_gpu_set_option(sparc_gpu_ctx *ctx, const char *key, int64_t value)
     if (!strcmp(key, "stencil_ty")) { ctx->opt_stencil_ty = (int)value; return 0; }
     if (!strcmp(key, "stencil_stages")) { ctx->opt_stencil_stages = (int)value; return 0; }
     if (!strcmp(key, "stencil_zchunks")) { ctx->opt_stencil_zchunks = (int)value; return 0; }
+    if (!strcmp(key, "nlb_tma")) { ctx->opt_nlb_tma = value ? 1 : 0; return 0; }
     if (!strcmp(key, "gemm_full")) { ctx->opt_gemm_full = value ? 1 : 0; return 0; }
     if (!strcmp(key, "gemm_path")) { if (value < 0 || value > 2) return SPARC_GPU_INVALID_ARG; ctx->opt_gemm_path = (int)value; return 0; }
     return SPARC_GPU_INVALID_ARG;

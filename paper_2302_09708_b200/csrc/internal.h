@@ -73,6 +73,7 @@ struct sparc_gpu_ctx {
     int opt_stencil_path;      // 0 auto, 1 generic, 2 TMA (DFMA), 3 TMA + DMMA in-plane taps
     int opt_nonlocal;          // 1 on
     int opt_gemm_path;         // 0 auto, 1 simple, 2 DMMA
+    int opt_nlb_tma;           // 0: brick kernel stages its tile with TMA; 1: direct global loads / stores
     int opt_gemm_full;         // 0: Hs, Ms computed as upper triangle + mirror (R12); 1: all tiles
     int opt_nonlocal_mode;     // 0 auto (brick kernel when supported, else 2), 1 project + pull (deterministic),
                                // 2 fused per-atom kernel with atomic scatter, 3 brick kernel or UNSUPPORTED

@@ -20,6 +20,10 @@
 //
 // The 9th projector of an s+p+d atom is applied as a rank-1 FMA update beside the two k-steps of DMMA (a third
 // k-step would be 3/4 padding).
+#include <cuda.h>
+
+#include <string.h>
+
 #include <algorithm>
 #include <unordered_map>
 #include <vector>
@@ -107,7 +111,25 @@ __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
     asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(smem_u32(bar)) : "memory");
 }
 
+__device__ __forceinline__ void tma_load_tile(void *dst, const CUtensorMap *tmap, uint64_t *bar, int x, int c, int y, int z)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(
+            smem_u32(dst)),
+        "l"(tmap), "r"(x), "r"(c), "r"(y), "r"(z), "r"(smem_u32(bar))
+        : "memory");
+}
+__device__ __forceinline__ void tma_store_tile(const CUtensorMap *tmap, const void *src, int x, int c, int y, int z)
+{
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%1, %2, %3, %4}], [%5];" ::"l"(tmap), "r"(x),
+                 "r"(c), "r"(y), "r"(z), "r"(smem_u32(src))
+                 : "memory");
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+
 constexpr int NLB_SLOTS = 16;                 // jobs in flight (mbarrier pairs)
+constexpr int NLB_TILE_BYTES = NB_PTS * NLB_COLS * 8;   // the 128 x 64 tile staged by TMA: [x-run][column][points of the run]
+constexpr int NLB_RING_TMA = 40 * 1024;       // ring size next to the staged tile (two CTAs per SM)
 constexpr int NLB_RING_BYTES = 72 * 1024;     // byte ring the producer warp streams chi blocks (+ C slices) through
 
 // KP: DMMA k-steps of the pull (projectors 0 .. 4 KP - 1); MT: 8-projector m-tiles of the projection; R1: projector
@@ -117,19 +139,25 @@ constexpr int NLB_RING_BYTES = 72 * 1024;     // byte ring the producer warp str
 // CTA's tile load / store overlaps the other's DMMAs): it walks the brick's job list ahead of the
 // consumers and streams, per (brick, atom) job, the chi blocks (and for a pull job the 64-column slice of C_J) into a
 // byte ring with cp.async.bulk; full/empty mbarriers per slot.
-template <int KP, int MT, bool R1, bool DO_PULL, bool DO_PROJ>
+// TMA_IO: the tile is loaded (and, after the pull, stored) by one TMA box copy through shared memory instead of 16
+// predicated 16-byte global accesses per lane: the tensor map orders the dimensions (x, column, y, z), so the box lands
+// as [x-run][column][points of the run] -- a warp's fragment read is then 512 contiguous bytes.
+template <int KP, int MT, bool R1, bool DO_PULL, bool DO_PROJ, bool TMA_IO>
 __global__ void __launch_bounds__((NLB_WARPS + 1) * 32, 2)
-nl_brick_kernel(const BrickParams p)
+nl_brick_kernel(const __grid_constant__ CUtensorMap tmap, const BrickParams p)
 {
     constexpr int PULL_SZ = KP * 32 + (R1 ? 8 : 0);
     constexpr int PROJ_SZ = MT * 64 + (R1 ? 8 : 0);
+    constexpr int RING_BYTES = TMA_IO ? NLB_RING_TMA : NLB_RING_BYTES;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    unsigned char *ring = smem_raw;                                                   // [NLB_RING_BYTES]
-    int32_t *pt_off = reinterpret_cast<int32_t *>(ring + NLB_RING_BYTES);             // [NB_PTS] grid index, -1 outside
+    unsigned char *tile = smem_raw;                                                   // [NLB_TILE_BYTES] (TMA_IO only)
+    unsigned char *ring = smem_raw + (TMA_IO ? NLB_TILE_BYTES : 0);                   // [RING_BYTES]
+    int32_t *pt_off = reinterpret_cast<int32_t *>(ring + RING_BYTES);                 // [NB_PTS] grid index, -1 outside
     uint64_t *full = reinterpret_cast<uint64_t *>(pt_off + NB_PTS);                   // [NLB_SLOTS]
     uint64_t *empty = full + NLB_SLOTS;                                               // [NLB_SLOTS]
     int4 *slot_info = reinterpret_cast<int4 *>(empty + NLB_SLOTS);                    // [NLB_SLOTS] offset, mask, P_J, po
     int32_t *slot_size = reinterpret_cast<int32_t *>(slot_info + NLB_SLOTS);          // [NLB_SLOTS] ring bytes (producer only)
+    uint64_t *tile_bar = reinterpret_cast<uint64_t *>(slot_size + NLB_SLOTS);         // tile landed (TMA_IO only)
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int lq = lane & 3, lr = lane >> 2;
@@ -137,13 +165,14 @@ nl_brick_kernel(const BrickParams p)
     const int cg = blockIdx.x - brick * p.ncolgroups;
     const int x0 = p.brick_org[4 * brick], y0 = p.brick_org[4 * brick + 1], z0 = p.brick_org[4 * brick + 2];
     const uint32_t umask = (uint32_t)p.brick_org[4 * brick + 3];
-    if (tid < NB_PTS) {
+    if (!TMA_IO && tid < NB_PTS) {
         const int lx = tid % p.bx, ly = (tid / p.bx) % p.by, lz = tid / (p.bx * p.by);
         const int x = x0 + lx, y = y0 + ly, z = z0 + lz;
         pt_off[tid] = (y < p.ny && z < p.nz) ? x + p.nx * (y + p.ny * z) : -1;
     }
     if (tid == 0) {
         for (int s = 0; s < NLB_SLOTS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NLB_WARPS); }
+        if (TMA_IO) mbar_init(tile_bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -155,6 +184,10 @@ nl_brick_kernel(const BrickParams p)
     if (warp == NLB_WARPS) {
         // ================================ producer warp ==========================================================
         // lanes fetch 32 job descriptors at a time; lane 0 allocates ring space in order and issues the copies
+        if (TMA_IO && lane == 0) {
+            mbar_expect_tx(tile_bar, (uint32_t)NLB_TILE_BYTES);
+            tma_load_tile(tile, &tmap, tile_bar, x0, cg * NLB_COLS, y0, z0);
+        }
         int head = 0, used = 0, freed = 0;
         for (int jb = 0; jb < njobs; jb += 32) {
             const int jmine = jb + lane;
@@ -172,9 +205,9 @@ nl_brick_kernel(const BrickParams p)
                 const uint32_t blk_bytes = (uint32_t)__popc(mask) * (uint32_t)(pull ? PULL_SZ : PROJ_SZ) * 8u;
                 const uint32_t c_bytes = pull ? (uint32_t)(NLB_COLS * pj * 8) : 0u;
                 int need = (int)((blk_bytes + c_bytes + 127u) & ~127u);
-                const bool wrap = head + need > NLB_RING_BYTES;                       // no job straddles the ring end
-                const int skip = wrap ? NLB_RING_BYTES - head : 0;
-                while (jj - freed >= NLB_SLOTS || used + need + skip > NLB_RING_BYTES) {
+                const bool wrap = head + need > RING_BYTES;                       // no job straddles the ring end
+                const int skip = wrap ? RING_BYTES - head : 0;
+                while (jj - freed >= NLB_SLOTS || used + need + skip > RING_BYTES) {
                     const int fs = freed % NLB_SLOTS;
                     mbar_wait(&empty[fs], (uint32_t)((freed / NLB_SLOTS) & 1));
                     used -= slot_size[fs];
@@ -207,7 +240,15 @@ nl_brick_kernel(const BrickParams p)
     const int32_t *pt_h = pt_off + 2 * lq;
     const double *srcc = p.src + (int64_t)(colv ? col : 0) * p.ld;
     double2 c[NB_HOCT];
-    {
+    // byte offset of this lane's pair of octet 0 inside the staged tile: [x-run][column][points of the run]
+    const int colL = (warp & 7) * 8 + lr;
+    // (an octet is 8 consecutive brick-local points = 8 / bx x-runs: octets are 8 x 64 x 8 = 4096 bytes apart)
+    const uint32_t toff0 = (uint32_t)(((((2 * lq) / p.bx) * NLB_COLS + colL) * p.bx + ((2 * lq) % p.bx)) * 8);
+    if (TMA_IO) {
+        mbar_wait(tile_bar, 0u);
+#pragma unroll
+        for (int o = 0; o < NB_HOCT; ++o) c[o] = *reinterpret_cast<const double2 *>(tile + toff0 + 4096 * o);
+    } else {
         // all offsets first, then branch-free loads: an untouched octet reads the column's first pair (a cached dummy)
         int off[NB_HOCT];
 #pragma unroll
@@ -270,14 +311,22 @@ nl_brick_kernel(const BrickParams p)
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[slot]);
             if (jj == na - 1) {                            // all atoms pulled: the tile is the final Out
-                double *dstc = p.dst + (int64_t)(colv ? col : 0) * p.ld;
-                int off[NB_HOCT];
+                if (TMA_IO) {
 #pragma unroll
-                for (int o = 0; o < NB_HOCT; ++o) off[o] = pt_h[8 * o];
+                    for (int o = 0; o < NB_HOCT; ++o) *reinterpret_cast<double2 *>(tile + toff0 + 4096 * o) = c[o];
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic writes -> async proxy
+                    asm volatile("bar.sync 1, %0;" ::"n"(NLB_WARPS * 32) : "memory");  // the eight consumer warps
+                    if (tid == 0) tma_store_tile(&tmap, tile, x0, cg * NLB_COLS, y0, z0);
+                } else {
+                    double *dstc = p.dst + (int64_t)(colv ? col : 0) * p.ld;
+                    int off[NB_HOCT];
 #pragma unroll
-                for (int o = 0; o < NB_HOCT; ++o) {
-                    const bool ok = ((umask_h >> o) & 1u) && off[o] >= 0 && colv;
-                    if (ok) *reinterpret_cast<double2 *>(dstc + off[o]) = c[o];
+                    for (int o = 0; o < NB_HOCT; ++o) off[o] = pt_h[8 * o];
+#pragma unroll
+                    for (int o = 0; o < NB_HOCT; ++o) {
+                        const bool ok = ((umask_h >> o) & 1u) && off[o] >= 0 && colv;
+                        if (ok) *reinterpret_cast<double2 *>(dstc + off[o]) = c[o];
+                    }
                 }
             }
         } else {
@@ -339,6 +388,8 @@ nl_brick_kernel(const BrickParams p)
             }
         }
     }
+    // the bulk store reads the staged tile asynchronously: it must be done before the CTA (and its shared memory) goes
+    if (TMA_IO && DO_PULL && tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
 struct ClassInfo { int kp, mt, r1, pull_sz, proj_sz; };
@@ -484,16 +535,36 @@ bool nlb_supported(const sparc_gpu_ctx *ctx, const double *X, int64_t ld)
 
 namespace {
 
-template <int KP, int MT, bool R1>
-int launch_class(sparc_gpu_ctx *ctx, int mode, const BrickParams &P, unsigned grid, cudaStream_t st)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// (x, column, y, z) tensor map over the N_d x ncols block with a bx x 64 x by x bz box: one brick x 64 columns
+bool encode_tile_map(const sparc_gpu_ctx *ctx, CUtensorMap *tm, const double *base, int64_t ld, int64_t ncols)
 {
-    constexpr size_t SMEM = (size_t)NLB_RING_BYTES + NB_PTS * 4 + NLB_SLOTS * (8 + 8 + 5 * 4);
-    void (*kern)(const BrickParams) = mode == 1 ? nl_brick_kernel<KP, MT, R1, false, true>
-                                      : mode == 2 ? nl_brick_kernel<KP, MT, R1, true, false>
-                                                  : nl_brick_kernel<KP, MT, R1, true, true>;
+    const NlBrick &B = ctx->nlb;
+    const int nx = ctx->n[0], ny = ctx->n[1], nz = ctx->n[2];
+    const cuuint64_t gdim[4] = {(cuuint64_t)nx, (cuuint64_t)ncols, (cuuint64_t)ny, (cuuint64_t)nz};
+    const cuuint64_t gstr[3] = {(cuuint64_t)ld * 8, (cuuint64_t)nx * 8, (cuuint64_t)nx * ny * 8};
+    const cuuint32_t box[4] = {(cuuint32_t)B.bx, (cuuint32_t)NLB_COLS, (cuuint32_t)B.by, (cuuint32_t)B.bz};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult cr = ((EncodeTiledFn)ctx->fn_encode_tiled)(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void *)base, gdim, gstr, box,
+                                                        estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                                        CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return cr == CUDA_SUCCESS;
+}
+
+template <int KP, int MT, bool R1, bool TMA_IO>
+int launch_class(sparc_gpu_ctx *ctx, int mode, const CUtensorMap &tmap, const BrickParams &P, unsigned grid, cudaStream_t st)
+{
+    constexpr size_t SMEM = (size_t)(TMA_IO ? NLB_TILE_BYTES + NLB_RING_TMA : NLB_RING_BYTES) + NB_PTS * 4 +
+                            NLB_SLOTS * (8 + 8 + 5 * 4) + 16;
+    void (*kern)(const CUtensorMap, const BrickParams) = mode == 1 ? nl_brick_kernel<KP, MT, R1, false, true, TMA_IO>
+                                                         : mode == 2 ? nl_brick_kernel<KP, MT, R1, true, false, TMA_IO>
+                                                                     : nl_brick_kernel<KP, MT, R1, true, true, TMA_IO>;
     SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
     prof_begin(ctx, KK_NL_BRICK, st);
-    kern<<<grid, (NLB_WARPS + 1) * 32, SMEM, st>>>(P);
+    kern<<<grid, (NLB_WARPS + 1) * 32, SMEM, st>>>(tmap, P);
     prof_end(ctx, KK_NL_BRICK, st);
     SPARC_CUDA_TRY(cudaGetLastError());
     return SPARC_GPU_SUCCESS;
@@ -521,7 +592,16 @@ int launch_nl_brick(sparc_gpu_ctx *ctx, int mode, double *XorOut, int64_t ld, in
     P.bx = B.bx; P.by = B.by; P.bz = B.bz;
     P.scale = scale;
     const unsigned grid = (unsigned)((int64_t)B.n_active * ngroups);
-    if (B.pclass == 4) SPARC_TRY((launch_class<1, 1, false>(ctx, mode, P, grid, st)));
-    else SPARC_TRY((launch_class<2, 1, true>(ctx, mode, P, grid, st)));
+    // tile staged by TMA when the driver entry point is there (option "nlb_tma" = 1 turns it off)
+    CUtensorMap tmap;
+    const bool tma = ctx->fn_encode_tiled && ctx->opt_nlb_tma != 1 && encode_tile_map(ctx, &tmap, XorOut, ld, ncols);
+    if (!tma) memset(&tmap, 0, sizeof(tmap));
+    if (B.pclass == 4) {
+        if (tma) SPARC_TRY((launch_class<1, 1, false, true>(ctx, mode, tmap, P, grid, st)));
+        else SPARC_TRY((launch_class<1, 1, false, false>(ctx, mode, tmap, P, grid, st)));
+    } else {
+        if (tma) SPARC_TRY((launch_class<2, 1, true, true>(ctx, mode, tmap, P, grid, st)));
+        else SPARC_TRY((launch_class<2, 1, true, false>(ctx, mode, tmap, P, grid, st)));
+    }
     return SPARC_GPU_SUCCESS;
 }

@@ -167,8 +167,10 @@ def test_brick_shapes_and_classes(torch, api, nx, projs):
     g.set_option("nonlocal_mode", 3)
     X = wl.psi_columns(range(wl.ns))
     H = orc.Hamiltonian(wl)
-    Yg = g.hamiltonian_apply(api.colmajor_from_numpy(X))
-    check_col(api.colmajor_to_numpy(Yg), H.apply(X), f"brick nx={nx} P={projs} H*Psi")
+    for tile_io in (1, 0):          # 1: direct global loads / stores of the tile, 0: staged by TMA (default)
+        g.set_option("nlb_tma", tile_io)
+        Yg = g.hamiltonian_apply(api.colmajor_from_numpy(X))
+        check_col(api.colmajor_to_numpy(Yg), H.apply(X), f"brick nx={nx} P={projs} H*Psi tile_io={tile_io}")
     for m, cb in ((1, 0), (4, 5)):
         Pg = api.colmajor_from_numpy(X)
         g.chebyshev_filter(Pg, m, wl.a, wl.b, wl.a0, col_block=cb)
