@@ -254,6 +254,7 @@ def run_ours(args):
     # largest share of the step, `roofline_by_kernel` lists the others.
     roofline = None
     rooflines = {}
+    filter_roofs = {"hbm_roof_units_per_s": 1.0, "fp64_roof_units_per_s": 1.0}
     kinds = {0: "stencil_generic", 1: "stencil_tma", 2: "nl_project", 3: "nl_pull", 4: "gemm_tn", 5: "gemm_nn",
              6: "splitk_reduce", 7: "copy2d", 8: "nl_fused", 9: "nl_brick"}
     share = {}
@@ -318,6 +319,12 @@ def run_ours(args):
         rooflines["gemm_nn"] = entry("gemm_nn", "tensor", prof_s[5][0], prof_s[5][1], g.get_info("gemm_nn_mflop") * 1e6,
                                      dmma_peak, "TFLOP/s", "measured now (sparc_gpu_probe_peak, FP64 DMMA)")
         rooflines = {k: v for k, v in rooflines.items() if v}
+        # the filter as a whole: 24 B and 2*(37+3) + 4*c*P flop per unit; the lower roof binds
+        flop_unit = 80.0 + 4.0 * supp_rows * pbar / nd
+        roof_hbm = hbm_peak * 1e9 / ALG_BYTES_PER_UNIT
+        roof_fp64 = dmma_peak * 1e12 / flop_unit
+        filter_roofs = {"flop_per_unit": flop_unit, "hbm_roof_units_per_s": roof_hbm, "fp64_roof_units_per_s": roof_fp64,
+                        "binding": "hbm" if roof_hbm <= roof_fp64 else "fp64"}
         roofline = dict(max(rooflines.values(), key=lambda e: e["share_of_step"]))
         roofline["filter_time_share_by_kernel"] = share
         roofline["fp64_peaks_tflops"] = {"dfma": dfma_peak, "dmma": dmma_peak}
@@ -364,6 +371,8 @@ def run_ours(args):
             "gpu_launches": int(launches),
             "roofline": roofline,
             "roofline_by_kernel": rooflines,
+            "filter_roofs": dict(filter_roofs, frac_of_binding=value / min(filter_roofs["hbm_roof_units_per_s"],
+                                                                             filter_roofs["fp64_roof_units_per_s"]) / world),
             "cpu_baseline": cpu_baseline,
         }
         print(json.dumps(line))
