@@ -21,10 +21,18 @@
  *     Hs, Ms, Q: ns x ns, column-major, ld = ns.
  *   - Pointers named *_dev are DEVICE pointers owned by the caller (e.g. PyTorch tensors); pointers in
  *     sparc_gpu_desc are HOST pointers, copied at create (the caller may free them afterwards).
- *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Every compute call
- *     is asynchronous on `stream`, never synchronises the device and never touches host memory.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Every operator call
+ *     (set_veff, hamiltonian_apply, chebyshev_filter, project, rotate, and the "next" operators below) is
+ *     asynchronous on `stream`, never synchronises the device and never touches host memory.  The
+ *     exceptions are support calls and say so: create / destroy (blocking uploads), sparc_gpu_probe_peak
+ *     (synchronises `stream`), sparc_gpu_get_info with a "prof_ns:<k>" key (waits for the recorded events)
+ *     and the *_host entry points (host buffers; they synchronise before returning).
+ *   - Every call makes ctx's device current for its duration and restores the caller's current device.
  *   - `ws_dev` is caller-owned device scratch of at least sparc_gpu_workspace_bytes(...) bytes, 256-byte
- *     aligned.  The library allocates only its immutable tables (weights, chi, index maps, Veff copy).
+ *     aligned.  The ABI carries no size with the pointer: declare it once with
+ *     sparc_gpu_set_workspace_size and every operator call that needs more returns WORKSPACE_TOO_SMALL
+ *     instead of overrunning the buffer.  The library allocates only its immutable tables (weights, chi,
+ *     index maps, Veff copy).
  *   - Every call returns 0 on success or a negative sparc_gpu_status.  No exceptions, no exit(), no
  *     printing.  There is NO CPU fallback: without an sm_100 device create fails with UNSUPPORTED.
  */
@@ -47,7 +55,7 @@ typedef enum {
     SPARC_GPU_BAD_BOUNDS = -3,          /* filter bounds must satisfy a0 < a < b (R5)                       */
     SPARC_GPU_BAD_DESCRIPTOR = -4,      /* support index out of range / not strictly ascending within an
                                            atom, inconsistent chi_ptr / supp_ptr, n_proj < 0 or > 16        */
-    SPARC_GPU_WORKSPACE_TOO_SMALL = -5, /* reserved: reported by bindings that know the size they passed    */
+    SPARC_GPU_WORKSPACE_TOO_SMALL = -5, /* the call needs more scratch than sparc_gpu_set_workspace_size declared */
     SPARC_GPU_OUT_OF_MEMORY = -6,       /* device allocation of the library's tables failed                 */
     SPARC_GPU_CUDA_ERROR = -7           /* any other CUDA runtime / driver error                            */
 } sparc_gpu_status;
@@ -92,6 +100,10 @@ int sparc_gpu_set_veff(sparc_gpu_ctx *ctx, const double *veff_dev, void *stream)
 int sparc_gpu_workspace_bytes(const sparc_gpu_ctx *ctx, int op, int64_t ns, int64_t block,
                               int64_t *bytes);
 
+/* Declare the size in bytes of the buffer that will be passed as `ws_dev` to the following calls on this context
+ * (0 = undeclared: no check, the caller vouches for sparc_gpu_workspace_bytes).  Host-side state only. */
+int sparc_gpu_set_workspace_size(sparc_gpu_ctx *ctx, int64_t bytes);
+
 /* Y = H X on ncols columns (eq. 4, 122-126).  X and Y must not overlap.
  * ldx, ldy >= N_d.  X is not modified. */
 int sparc_gpu_hamiltonian_apply(sparc_gpu_ctx *ctx, const double *X_dev, int64_t ldx, double *Y_dev,
@@ -134,19 +146,30 @@ int sparc_gpu_fill_uniform(double *dst_dev, int64_t count, uint64_t seed, uint64
 int sparc_gpu_probe_peak(int device, int kind, double *value_out, void *scratch_dev, int64_t scratch_bytes,
                          void *stream);
 
-/* Tuning / test knobs.  key: "stencil_path" (0 auto, 1 generic kernel, 2 TMA + DFMA kernel, 3 TMA + DMMA in-plane
- * taps; 2 and 3 return UNSUPPORTED from the operator call when the grid does not meet their preconditions),
- * "nonlocal" (1 on, 0 off: drops V_nl, used by closed-form pins), "nonlocal_mode" (0 auto = brick-tiled DMMA kernel
- * when supported, 1 project + pull: bitwise reproducible, 2 per-atom fused kernel with atomic scatter, 3 brick kernel
- * or UNSUPPORTED), "gemm_path" (0 auto, 1 simple FMA kernel, 2 DMMA kernel), "profile" / "profile_reset" (per-kernel
- * CUDA-event timing read back through sparc_gpu_get_info "prof_ns:<kind>" / "prof_count:<kind>"), "nlb_tma" (0: the brick
- * kernel stages its tile with TMA, 1: direct global loads / stores), "gemm_full" (0: Hs, Ms as upper-triangle tiles +
- * mirror, 1: all tiles), and the stencil tile knobs "stencil_ay", "stencil_ty", "stencil_stages", "stencil_zchunks" (0 = library chooses).
- * Unknown key -> INVALID_ARG. */
+/* Tuning / test knobs (host-side state of the context; unknown key or out-of-range value -> INVALID_ARG).
+ *   "stencil_path"    0 auto, 1 generic kernel, 2 TMA + DFMA kernel, 3 TMA + DMMA in-plane taps; 2 and 3 make the
+ *                     operator call return UNSUPPORTED when the grid does not meet their preconditions
+ *   "nonlocal"        1 on, 0 off: drops V_nl (used by closed-form pins)
+ *   "nonlocal_mode"   0 auto (brick-tiled DMMA kernel when supported, else 2), 1 project + pull: bitwise reproducible,
+ *                     2 per-atom kernel with atomic scatter, 3 brick kernel or UNSUPPORTED
+ *   "nlb_variant"     brick kernel shape: 0 = 32 columns per CTA, three CTAs per SM; 1 = 32 columns, four CTAs;
+ *                     2 = 64 columns, two CTAs
+ *   "gemm_path"       0 auto, 1 simple FMA kernel, 2 DMMA kernel
+ *   "gemm_full"       0: Hs, Ms as upper-triangle tiles + mirror (R12), 1: all tiles
+ *   "stencil_ay" (0 auto, 1, 2), "stencil_ty" (0 auto, else tile rows), "stencil_stages" (0 auto, 2..8 TMA ring depth),
+ *   "stencil_zchunks" (0 auto): tile knobs of the stencil kernels
+ *   "profile" (0 / 1), "profile_reset": per-kernel CUDA-event timing, read back through sparc_gpu_get_info */
 int sparc_gpu_set_option(sparc_gpu_ctx *ctx, const char *key, int64_t value);
 
-/* Read-only counters / facts.  key: "kernel_launches" (cumulative kernels launched by this context),
- * "nd", "n_proj_total", "covered_points", "stencil_path_last" (1 generic, 2 TMA), "sm_count". */
+/* Read-only counters / facts.  key:
+ *   "kernel_launches" (cumulative kernels launched by this context), "nd", "n_proj_total", "covered_points", "sm_count",
+ *   "stencil_path_last" (1 generic, 2 TMA + DFMA, 3 TMA + DMMA hybrid: the kernel the last local pass used),
+ *   "nl_brick" (1: the brick tables exist), "nl_brick_blocks", "nl_brick_active" (chi blocks / bricks with work),
+ *   "gemm_tn_mflop", "gemm_nn_mflop" (flop issued by the DMMA GEMMs since the last "profile_reset", in 1e6),
+ *   "prof_count:<k>" launches and "prof_ns:<k>" summed nanoseconds of kernel kind k since the last "profile_reset"
+ *   (k: 0 generic stencil, 1 TMA stencils, 2 nl project, 3 nl pull, 4 GEMM TN, 5 GEMM NN, 6 split-K reduce, 7 copies /
+ *   mirror, 8 per-atom nonlocal, 9 brick nonlocal, 10 gradient stencil, 11 eigensolver kernels).  "prof_ns:<k>" waits for
+ *   the recorded events (cudaEventSynchronize): the one get_info key that blocks. */
 int sparc_gpu_get_info(const sparc_gpu_ctx *ctx, const char *key, int64_t *value);
 
 const char *sparc_gpu_error_string(int code);

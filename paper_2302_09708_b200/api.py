@@ -23,6 +23,7 @@ _lib = None
 OP_HAMILTONIAN_APPLY, OP_CHEBYSHEV_FILTER, OP_PROJECT, OP_ROTATE = 0, 1, 2, 3
 
 EXPORTS = ["sparc_gpu_create", "sparc_gpu_destroy", "sparc_gpu_set_veff", "sparc_gpu_workspace_bytes",
+           "sparc_gpu_set_workspace_size",
            "sparc_gpu_hamiltonian_apply", "sparc_gpu_chebyshev_filter", "sparc_gpu_project",
            "sparc_gpu_rotate", "sparc_gpu_fill_uniform", "sparc_gpu_set_option", "sparc_gpu_get_info", "sparc_gpu_probe_peak",
            "sparc_gpu_error_string", "sparc_gpu_version"]
@@ -59,6 +60,7 @@ def load_library(build_if_missing: bool = True):
     lib.sparc_gpu_destroy.argtypes = [P]
     lib.sparc_gpu_set_veff.argtypes = [P, P, P]
     lib.sparc_gpu_workspace_bytes.argtypes = [P, I, I64, I64, C.POINTER(I64)]
+    lib.sparc_gpu_set_workspace_size.argtypes = [P, I64]
     lib.sparc_gpu_hamiltonian_apply.argtypes = [P, P, I64, P, I64, I64, P, P]
     lib.sparc_gpu_chebyshev_filter.argtypes = [P, P, I64, I64, I, D, D, D, I64, P, P]
     lib.sparc_gpu_project.argtypes = [P, P, I64, I64, P, P, I64, P, P]
@@ -86,8 +88,9 @@ def _torch():
     return torch
 
 
-def _stream_ptr():
-    return C.c_void_p(_torch().cuda.current_stream().cuda_stream)
+def _stream_ptr(device=None):
+    """cudaStream_t of torch's current stream ON `device` (not on whatever device happens to be current)."""
+    return C.c_void_p(_torch().cuda.current_stream(device).cuda_stream)
 
 
 def colmajor_from_numpy(a: np.ndarray, device="cuda", ld: Optional[int] = None):
@@ -112,7 +115,7 @@ def fill_uniform(t, seed: int, stream_id: int, index0: int, lo: float, hi: float
     """t.view(-1)[k] = lo + (hi-lo)*u(seed, stream_id, index0+k) on the device (contiguous tensor)."""
     assert t.is_cuda and t.is_contiguous() and t.dtype == _torch().float64
     _check(load_library().sparc_gpu_fill_uniform(C.c_void_p(t.data_ptr()), t.numel(), seed, stream_id, index0,
-                                                 lo, hi, t.device.index or 0, _stream_ptr()), "fill_uniform")
+                                                 lo, hi, t.device.index or 0, _stream_ptr(t.device)), "fill_uniform")
     return t
 
 
@@ -122,7 +125,7 @@ def probe_peak(kind: int, device: int = 0, scratch_bytes: int = 1 << 30) -> floa
     scratch = torch.empty(scratch_bytes if kind == 2 else 4096, dtype=torch.uint8, device=f"cuda:{device}")
     out = C.c_double()
     _check(load_library().sparc_gpu_probe_peak(int(device), int(kind), C.byref(out), C.c_void_p(scratch.data_ptr()),
-                                               scratch.numel(), _stream_ptr()), "probe_peak")
+                                               scratch.numel(), _stream_ptr(scratch.device)), "probe_peak")
     return out.value
 
 
@@ -188,10 +191,17 @@ class SparcGpu:
         if self._ws is None or self._ws.numel() < need:
             self._ws = None
             self._ws = torch.empty(need, dtype=torch.uint8, device=f"cuda:{self.device}")
+            # the ABI carries no size with ws_dev: declare it, so that a short buffer is an error code, not an overrun
+            _check(self.lib.sparc_gpu_set_workspace_size(self._ctx, self._ws.numel()), "set_workspace_size")
         return C.c_void_p(self._ws.data_ptr())
 
     def release_workspace(self):
         self._ws = None
+        if getattr(self, "_ctx", None) is not None and self._ctx.value:
+            self.lib.sparc_gpu_set_workspace_size(self._ctx, 0)
+
+    def _stream(self):
+        return _stream_ptr(self.device)
 
     def set_option(self, key: str, value: int):
         _check(self.lib.sparc_gpu_set_option(self._ctx, key.encode(), int(value)), f"set_option({key})")
@@ -212,7 +222,7 @@ class SparcGpu:
     # ---- the C-ABI calls ----------------------------------------------------------------------
     def set_veff(self, veff):
         assert veff.is_cuda and veff.numel() >= self.nd and veff.is_contiguous()
-        _check(self.lib.sparc_gpu_set_veff(self._ctx, C.c_void_p(veff.data_ptr()), _stream_ptr()), "set_veff")
+        _check(self.lib.sparc_gpu_set_veff(self._ctx, C.c_void_p(veff.data_ptr()), self._stream()), "set_veff")
 
     def hamiltonian_apply(self, X, Y=None):
         torch = _torch()
@@ -221,7 +231,7 @@ class SparcGpu:
             Y = torch.empty_like(X)
         yp, ldy, _ = self._mat(Y, "Y")
         ws = self._workspace(OP_HAMILTONIAN_APPLY, ncols, 0)
-        _check(self.lib.sparc_gpu_hamiltonian_apply(self._ctx, xp, ldx, yp, ldy, ncols, ws, _stream_ptr()),
+        _check(self.lib.sparc_gpu_hamiltonian_apply(self._ctx, xp, ldx, yp, ldy, ncols, ws, self._stream()),
                "hamiltonian_apply")
         return Y
 
@@ -229,7 +239,7 @@ class SparcGpu:
         pp, ld, ns = self._mat(Psi, "Psi")
         ws = self._workspace(OP_CHEBYSHEV_FILTER, ns, col_block)
         _check(self.lib.sparc_gpu_chebyshev_filter(self._ctx, pp, ld, ns, int(degree), float(a), float(b),
-                                                   float(a0), int(col_block), ws, _stream_ptr()),
+                                                   float(a0), int(col_block), ws, self._stream()),
                "chebyshev_filter")
         return Psi
 
@@ -291,7 +301,7 @@ class SparcGpu:
             Ms = torch.empty((ns, ns), dtype=torch.float64, device=Psi.device)
         ws = self._workspace(OP_PROJECT, ns, col_block)
         _check(self.lib.sparc_gpu_project(self._ctx, pp, ld, ns, C.c_void_p(Hs.data_ptr()),
-                                          C.c_void_p(Ms.data_ptr()), int(col_block), ws, _stream_ptr()), "project")
+                                          C.c_void_p(Ms.data_ptr()), int(col_block), ws, self._stream()), "project")
         return Hs, Ms       # (ns, ns) tensors holding the column-major matrices: element [j, i] = M_ij
 
     def rotate(self, Psi, Q, row_panel: int = 0):
@@ -299,5 +309,5 @@ class SparcGpu:
         assert Q.is_cuda and Q.shape == (ns, ns) and Q.is_contiguous()
         ws = self._workspace(OP_ROTATE, ns, row_panel)
         _check(self.lib.sparc_gpu_rotate(self._ctx, pp, ld, ns, C.c_void_p(Q.data_ptr()), int(row_panel), ws,
-                                         _stream_ptr()), "rotate")
+                                         self._stream()), "rotate")
         return Psi

@@ -184,6 +184,12 @@ int ws_layout(const sparc_gpu_ctx *c, int op, int64_t ns, int64_t block, WsLayou
     return SPARC_GPU_SUCCESS;
 }
 
+// the caller declared the size of its workspace (sparc_gpu_set_workspace_size): refuse a call that would overrun it
+int ws_check(const sparc_gpu_ctx *c, const WsLayout &L)
+{
+    return (c->ws_bytes > 0 && L.total > c->ws_bytes) ? SPARC_GPU_WORKSPACE_TOO_SMALL : SPARC_GPU_SUCCESS;
+}
+
 // Out = alpha (H_loc X + shift X) + beta Prev on one column block: the fused local pass (stencil + Veff + axpy).
 int local_pass(sparc_gpu_ctx *c, const double *X, int64_t ldx, double *Out, int64_t ldo, const double *Prev,
                int64_t ldp, int64_t ncols, double alpha, double shift, double beta, cudaStream_t st)
@@ -273,17 +279,16 @@ int sparc_gpu_create(const sparc_gpu_desc *desc, sparc_gpu_ctx **out)
     cudaDeviceProp prop;
     SPARC_CUDA_TRY(cudaGetDeviceProperties(&prop, desc->device));
     if (prop.major != 10) return SPARC_GPU_UNSUPPORTED;     // sm_100a only, no fallback
-    SPARC_CUDA_TRY(cudaSetDevice(desc->device));
+    DeviceGuard dg(desc->device);
+    if (!dg.ok) return SPARC_GPU_CUDA_ERROR;
 
     sparc_gpu_ctx *c = new (std::nothrow) sparc_gpu_ctx();
     if (!c) return SPARC_GPU_OUT_OF_MEMORY;
-    memset(c, 0, sizeof(*c));
     c->device = desc->device;
     c->sm_count = prop.multiProcessorCount;
     for (int a = 0; a < 3; ++a) { c->n[a] = desc->n[a]; c->h[a] = desc->h[a]; c->bc[a] = desc->bc[a]; }
     c->radius = desc->fd_order / 2;
     c->nd = (int64_t)desc->n[0] * desc->n[1] * desc->n[2];
-    c->opt_nonlocal = 1;
     c->prof = new (std::nothrow) ProfState();
     fd_weights_host(c->radius, c->w);
     double isum = 0.0;
@@ -373,7 +378,7 @@ int sparc_gpu_create(const sparc_gpu_desc *desc, sparc_gpu_ctx **out)
 int sparc_gpu_destroy(sparc_gpu_ctx *ctx)
 {
     if (!ctx) return SPARC_GPU_INVALID_ARG;
-    cudaSetDevice(ctx->device);
+    DeviceGuard dg(ctx->device);
     free_tables(ctx);
     if (ctx->prof) {
         prof_collect(ctx->prof);
@@ -387,6 +392,8 @@ int sparc_gpu_destroy(sparc_gpu_ctx *ctx)
 int sparc_gpu_set_veff(sparc_gpu_ctx *ctx, const double *veff_dev, void *stream)
 {
     if (!ctx || !veff_dev) return SPARC_GPU_INVALID_ARG;
+    DeviceGuard dg(ctx->device);
+    if (!dg.ok) return SPARC_GPU_CUDA_ERROR;
     SPARC_CUDA_TRY(cudaMemcpyAsync(ctx->d_veff, veff_dev, (size_t)ctx->nd * 8, cudaMemcpyDeviceToDevice,
                                    (cudaStream_t)stream));
     return SPARC_GPU_SUCCESS;
@@ -406,11 +413,14 @@ int sparc_gpu_set_option(sparc_gpu_ctx *ctx, const char *key, int64_t value)
         ctx->gemm_flop[0] = ctx->gemm_flop[1] = 0.0;
         return 0;
     }
-    if (!strcmp(key, "stencil_ay")) { ctx->opt_stencil_ay = (int)value; return 0; }
-    if (!strcmp(key, "stencil_ty")) { ctx->opt_stencil_ty = (int)value; return 0; }
-    if (!strcmp(key, "stencil_stages")) { ctx->opt_stencil_stages = (int)value; return 0; }
-    if (!strcmp(key, "stencil_zchunks")) { ctx->opt_stencil_zchunks = (int)value; return 0; }
-    if (!strcmp(key, "nlb_tma")) { ctx->opt_nlb_tma = value ? 1 : 0; return 0; }
+    if (!strcmp(key, "stencil_ay")) { if (value < 0 || value > 2) return SPARC_GPU_INVALID_ARG; ctx->opt_stencil_ay = (int)value; ctx->tma_choice.valid = 0; return 0; }
+    if (!strcmp(key, "stencil_ty")) { if (value < 0) return SPARC_GPU_INVALID_ARG; ctx->opt_stencil_ty = (int)value; ctx->tma_choice.valid = 0; return 0; }
+    // ring depth 2..8 (a one-stage ring cannot overlap the TMA copy with the arithmetic: rejected here, not at launch)
+    if (!strcmp(key, "stencil_stages")) { if (value != 0 && (value < 2 || value > 8)) return SPARC_GPU_INVALID_ARG; ctx->opt_stencil_stages = (int)value; ctx->tma_choice.valid = 0; return 0; }
+    if (!strcmp(key, "stencil_zchunks")) { if (value < 0) return SPARC_GPU_INVALID_ARG; ctx->opt_stencil_zchunks = (int)value; return 0; }
+    if (!strcmp(key, "nlb_dbg")) { ctx->opt_nlb_dbg = (int)value; return 0; }
+    if (!strcmp(key, "nlb_kernel")) { if (value < 0 || value > 2) return SPARC_GPU_INVALID_ARG; ctx->opt_nlb_kernel = (int)value; return 0; }
+    if (!strcmp(key, "nlb_cap")) { if (value < 0) return SPARC_GPU_INVALID_ARG; ctx->opt_nlb_cap = (int)value; return 0; }
     if (!strcmp(key, "gemm_full")) { ctx->opt_gemm_full = value ? 1 : 0; return 0; }
     if (!strcmp(key, "gemm_path")) { if (value < 0 || value > 2) return SPARC_GPU_INVALID_ARG; ctx->opt_gemm_path = (int)value; return 0; }
     return SPARC_GPU_INVALID_ARG;
@@ -442,6 +452,13 @@ int sparc_gpu_get_info(const sparc_gpu_ctx *ctx, const char *key, int64_t *value
     return SPARC_GPU_INVALID_ARG;
 }
 
+int sparc_gpu_set_workspace_size(sparc_gpu_ctx *ctx, int64_t bytes)
+{
+    if (!ctx || bytes < 0) return SPARC_GPU_INVALID_ARG;
+    ctx->ws_bytes = bytes;
+    return SPARC_GPU_SUCCESS;
+}
+
 int sparc_gpu_workspace_bytes(const sparc_gpu_ctx *ctx, int op, int64_t ns, int64_t block, int64_t *bytes)
 {
     if (!ctx || !bytes) return SPARC_GPU_INVALID_ARG;
@@ -457,9 +474,11 @@ int sparc_gpu_hamiltonian_apply(sparc_gpu_ctx *ctx, const double *X, int64_t ldx
     if (!ctx || ncols < 0) return SPARC_GPU_INVALID_ARG;
     if (ncols == 0) return SPARC_GPU_SUCCESS;
     if (!X || !Y || !ws || ldx < ctx->nd || ldy < ctx->nd) return SPARC_GPU_INVALID_ARG;
-    SPARC_CUDA_TRY(cudaSetDevice(ctx->device));
+    DeviceGuard dg(ctx->device);
+    if (!dg.ok) return SPARC_GPU_CUDA_ERROR;
     WsLayout L;
     SPARC_TRY(ws_layout(ctx, SPARC_GPU_OP_HAMILTONIAN_APPLY, ncols, 0, &L));
+    SPARC_TRY(ws_check(ctx, L));
     double *D = (double *)((char *)ws + L.off_d);
     for (int64_t j0 = 0; j0 < ncols; j0 += L.block) {
         const int64_t nb = std::min(L.block, ncols - j0);
@@ -475,10 +494,12 @@ int sparc_gpu_chebyshev_filter(sparc_gpu_ctx *ctx, double *Psi, int64_t ld, int6
     if (!(a0 < a && a < b)) return SPARC_GPU_BAD_BOUNDS;
     if (ns == 0 || degree == 0) return SPARC_GPU_SUCCESS;
     if (!Psi || !ws || ld < ctx->nd) return SPARC_GPU_INVALID_ARG;
-    SPARC_CUDA_TRY(cudaSetDevice(ctx->device));
+    DeviceGuard dg(ctx->device);
+    if (!dg.ok) return SPARC_GPU_CUDA_ERROR;
     cudaStream_t st = (cudaStream_t)stream;
     WsLayout L;
     SPARC_TRY(ws_layout(ctx, SPARC_GPU_OP_CHEBYSHEV_FILTER, ns, col_block, &L));
+    SPARC_TRY(ws_check(ctx, L));
     double *W = (double *)((char *)ws + L.off_w);
     double *D = (double *)((char *)ws + L.off_d);
     const double e = 0.5 * (b - a), c = 0.5 * (b + a);
@@ -524,10 +545,12 @@ int sparc_gpu_project(sparc_gpu_ctx *ctx, const double *Psi, int64_t ld, int64_t
     if (!ctx || ns < 0) return SPARC_GPU_INVALID_ARG;
     if (ns == 0) return SPARC_GPU_SUCCESS;
     if (!Psi || !Hs || !Ms || !ws || ld < ctx->nd) return SPARC_GPU_INVALID_ARG;
-    SPARC_CUDA_TRY(cudaSetDevice(ctx->device));
+    DeviceGuard dg(ctx->device);
+    if (!dg.ok) return SPARC_GPU_CUDA_ERROR;
     cudaStream_t st = (cudaStream_t)stream;
     WsLayout L;
     SPARC_TRY(ws_layout(ctx, SPARC_GPU_OP_PROJECT, ns, col_block, &L));
+    SPARC_TRY(ws_check(ctx, L));
     double *Y = (double *)((char *)ws + L.off_w);
     double *D = (double *)((char *)ws + L.off_d);
     void *G = (char *)ws + L.off_g;
@@ -553,10 +576,12 @@ int sparc_gpu_rotate(sparc_gpu_ctx *ctx, double *Psi, int64_t ld, int64_t ns, co
     if (!ctx || ns < 0) return SPARC_GPU_INVALID_ARG;
     if (ns == 0) return SPARC_GPU_SUCCESS;
     if (!Psi || !Q || !ws || ld < ctx->nd) return SPARC_GPU_INVALID_ARG;
-    SPARC_CUDA_TRY(cudaSetDevice(ctx->device));
+    DeviceGuard dg(ctx->device);
+    if (!dg.ok) return SPARC_GPU_CUDA_ERROR;
     cudaStream_t st = (cudaStream_t)stream;
     WsLayout L;
     SPARC_TRY(ws_layout(ctx, SPARC_GPU_OP_ROTATE, ns, row_panel, &L));
+    SPARC_TRY(ws_check(ctx, L));
     double *T = (double *)((char *)ws + L.off_w);
     for (int64_t r0 = 0; r0 < ctx->nd; r0 += L.block) {
         const int64_t nr = std::min(L.block, ctx->nd - r0);

@@ -28,7 +28,8 @@ extern "C" int sparc_gpu_fill_uniform(double *dst_dev, int64_t count, uint64_t s
 {
     if (count < 0 || (count > 0 && !dst_dev)) return SPARC_GPU_INVALID_ARG;
     if (count == 0) return SPARC_GPU_SUCCESS;
-    SPARC_CUDA_TRY(cudaSetDevice(device));
+    DeviceGuard dg(device);
+    if (!dg.ok) return SPARC_GPU_CUDA_ERROR;
     const uint64_t key = mix64(seed * 0xD1B54A32D192ED03ULL + stream_id * 0x8CB92BA72F3D8DD7ULL + 0x9E3779B97F4A7C15ULL);
     int64_t blocks = (count + 255) / 256;
     if (blocks > 148 * 16) blocks = 148 * 16;

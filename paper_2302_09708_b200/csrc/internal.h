@@ -35,66 +35,95 @@ struct NlBrick {
     int32_t *d_org = nullptr;      // [n_active][4]: x0, y0, z0, union octet mask
     int32_t *d_job_ptr = nullptr;  // [n_active + 1]
     void *d_jobs = nullptr;        // BrickJob[]
-    double *d_pull = nullptr;      // pull-fragment blocks
-    double *d_proj = nullptr;      // projection-fragment blocks
+    int64_t max_blocks = 0;        // most chi blocks any one brick has
+    int64_t max_jobs = 0;          // most atoms meeting any one brick
+    double *d_blk = nullptr;       // chi sqrt|gamma| blocks, one copy serving pull and projection
+};
+
+// Tile choice of the TMA stencil kernel (stencil_tma.cu): depends only on the grid, the boundary flags and the
+// "stencil_*" options, so it is computed once per context and invalidated by sparc_gpu_set_option.
+struct StencilTileChoice {
+    int valid = 0;             // 0: not computed yet, 1: usable, -1: no tile fits (kernel unsupported on this grid)
+    int AY = 0, TY = 0, threads = 0, ctas_per_sm = 0, nstage = 0, W = 0, variant = 0;
+    uint32_t psi_bytes = 0, tile_bytes = 0, stage_bytes = 0;
+    size_t smem = 0;
 };
 
 struct sparc_gpu_ctx {
-    int device;
-    int sm_count;
-    int32_t n[3];
-    double h[3];
-    int32_t bc[3];
-    int32_t radius;
-    int64_t nd;
-    StencilCoef coef;          // alpha = 1 coefficients (host copy)
-    double w[SPARC_MAX_RADIUS + 1];
+    int device = 0;
+    int sm_count = 0;
+    int32_t n[3] = {0, 0, 0};
+    double h[3] = {0, 0, 0};
+    int32_t bc[3] = {0, 0, 0};
+    int32_t radius = 0;
+    int64_t nd = 0;
+    StencilCoef coef = {};     // alpha = 1 coefficients (host copy)
+    double w[SPARC_MAX_RADIUS + 1] = {0};
+    double w1[SPARC_MAX_RADIUS + 1] = {0};   // first-derivative weights (gradient stencil, forces)
     // nonlocal tables (device)
-    int32_t n_atoms;
-    int32_t n_proj_total;
-    int32_t max_proj;
-    int64_t supp_total;
-    int64_t *d_supp_ptr;       // [n_atoms+1]
-    int32_t *d_supp_idx;       // [supp_total]
-    int32_t *d_n_proj;         // [n_atoms]
-    int32_t *d_proj_ofs;       // [n_atoms+1] prefix sum of n_proj
-    int64_t *d_chi_ptr;        // [n_atoms+1]
-    double *d_chi;
-    double *d_gamma;           // [n_proj_total]
+    int32_t n_atoms = 0;
+    int32_t n_proj_total = 0;
+    int32_t max_proj = 0;
+    int64_t supp_total = 0;
+    int64_t *d_supp_ptr = nullptr;       // [n_atoms+1]
+    int32_t *d_supp_idx = nullptr;       // [supp_total]
+    int32_t *d_n_proj = nullptr;         // [n_atoms]
+    int32_t *d_proj_ofs = nullptr;       // [n_atoms+1] prefix sum of n_proj
+    int64_t *d_chi_ptr = nullptr;        // [n_atoms+1]
+    double *d_chi = nullptr;
+    double *d_gamma = nullptr;           // [n_proj_total]
     // inverse (pull) map
-    int64_t n_covered;
-    int32_t *d_cov_idx;        // [n_covered] grid index of each covered point (ascending)
-    int64_t *d_cov_ptr;        // [n_covered+1] offsets into d_cov_ent
-    CoverEntry *d_cov_ent;     // [supp_total]
+    int64_t n_covered = 0;
+    int32_t *d_cov_idx = nullptr;        // [n_covered] grid index of each covered point (ascending)
+    int64_t *d_cov_ptr = nullptr;        // [n_covered+1] offsets into d_cov_ent
+    CoverEntry *d_cov_ent = nullptr;     // [supp_total]
     NlBrick nlb;
     // local potential
-    double *d_veff;            // [nd]
+    double *d_veff = nullptr;            // [nd]
     // options
-    int opt_stencil_path;      // 0 auto, 1 generic, 2 TMA (DFMA), 3 TMA + DMMA in-plane taps
-    int opt_nonlocal;          // 1 on
-    int opt_gemm_path;         // 0 auto, 1 simple, 2 DMMA
-    int opt_nlb_tma;           // 0: brick kernel stages its tile with TMA; 1: direct global loads / stores
-    int opt_gemm_full;         // 0: Hs, Ms computed as upper triangle + mirror (R12); 1: all tiles
-    int opt_nonlocal_mode;     // 0 auto (brick kernel when supported, else 2), 1 project + pull (deterministic),
-                               // 2 fused per-atom kernel with atomic scatter, 3 brick kernel or UNSUPPORTED
-    int opt_stencil_ay;        // 0 auto, 1 or 2: rows per consumer thread of the TMA stencil kernel
-    int opt_stencil_ty;        // 0 auto, else forced tile rows of the TMA stencil kernel
-    int opt_stencil_stages;    // 0 auto, else cap on the smem ring depth
-    int opt_stencil_zchunks;   // 0 auto, else forced number of z chunks
+    int opt_stencil_path = 0;      // 0 auto, 1 generic, 2 TMA (DFMA), 3 TMA + DMMA in-plane taps
+    int opt_nonlocal = 1;          // 1 on
+    int opt_gemm_path = 0;         // 0 auto, 1 simple, 2 DMMA
+    int opt_nlb_kernel = 0;        // brick kernel: 0 auto (persistent when every brick fits its store), 1 general, 2 persistent
+    int opt_nlb_cap = 0;           // test knob: cap on the chi blocks the brick kernel keeps in shared memory (0 = all that fit)
+    int opt_nlb_dbg = 0;           // timing experiments (nonlocal_brick.cu)
+    int opt_gemm_full = 0;         // 0: Hs, Ms computed as upper triangle + mirror (R12); 1: all tiles
+    int opt_nonlocal_mode = 0;     // 0 auto (brick kernel when supported, else 2), 1 project + pull (deterministic),
+                                   // 2 per-atom kernel with atomic scatter, 3 brick kernel or UNSUPPORTED
+    int opt_stencil_ay = 0;        // 0 auto, 1 or 2: rows per consumer thread of the TMA stencil kernel
+    int opt_stencil_ty = 0;        // 0 auto, else forced tile rows of the TMA stencil kernel
+    int opt_stencil_stages = 0;    // 0 auto, else cap on the smem ring depth (2..8)
+    int opt_stencil_zchunks = 0;   // 0 auto, else forced number of z chunks
+    // size of the buffer the caller passes as ws_dev (sparc_gpu_set_workspace_size); 0 = not declared, no check
+    int64_t ws_bytes = 0;
     // counters
-    mutable int64_t kernel_launches;
-    double gemm_flop[2];       // flop issued by the DMMA GEMMs since the last "profile_reset": [0] TN, [1] NN
-    int stencil_path_last;
+    mutable int64_t kernel_launches = 0;
+    double gemm_flop[2] = {0, 0};  // flop issued by the DMMA GEMMs since the last "profile_reset": [0] TN, [1] NN
+    int stencil_path_last = 0;
+    mutable StencilTileChoice tma_choice;  // cache (stencil_tma.cu)
+    uint64_t func_attr_done = 0;   // kernel variants whose dynamic shared-memory attribute is set (nonlocal_brick.cu)
     // driver entry point for tensor-map encoding (resolved at create; NULL if unavailable)
-    void *fn_encode_tiled;
+    void *fn_encode_tiled = nullptr;
     // optional per-kernel CUDA-event timing (option "profile"); NULL when off
-    struct ProfState *prof;
+    struct ProfState *prof = nullptr;
+};
+
+// Make ctx->device current for the duration of a C-ABI call and restore the caller's device afterwards.
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { (void)cudaGetLastError(); prev = -1; }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) { (void)cudaGetLastError(); ok = false; }
+    }
+    ~DeviceGuard() { if (prev >= 0) (void)cudaSetDevice(prev); }
 };
 
 // Kernel kinds for the event profiler and the launch counters.
 enum KernelKind {
     KK_STENCIL_GENERIC = 0, KK_STENCIL_TMA = 1, KK_NL_PROJECT = 2, KK_NL_PULL = 3, KK_GEMM_TN = 4,
-    KK_GEMM_NN = 5, KK_SPLITK_REDUCE = 6, KK_COPY2D = 7, KK_NL_FUSED = 8, KK_NL_BRICK = 9, KK_COUNT = 10
+    KK_GEMM_NN = 5, KK_SPLITK_REDUCE = 6, KK_COPY2D = 7, KK_NL_FUSED = 8, KK_NL_BRICK = 9, KK_GRADIENT = 10, KK_EIG = 11, KK_COUNT = 12
 };
 // Bracket one kernel launch with events when profiling is on (no-ops otherwise); both bump the counters.
 void prof_begin(sparc_gpu_ctx *ctx, int kind, cudaStream_t st);

@@ -58,7 +58,8 @@ extern "C" int sparc_gpu_probe_peak(int device, int kind, double *value_out, voi
 {
     if (!value_out || kind < 0 || kind > 2) return SPARC_GPU_INVALID_ARG;
     if (!scratch_dev || scratch_bytes < 64) return SPARC_GPU_WORKSPACE_TOO_SMALL;
-    SPARC_CUDA_TRY(cudaSetDevice(device));
+    DeviceGuard dg(device);
+    if (!dg.ok) return SPARC_GPU_CUDA_ERROR;
     cudaDeviceProp prop;
     SPARC_CUDA_TRY(cudaGetDeviceProperties(&prop, device));
     if (prop.major != 10) return SPARC_GPU_UNSUPPORTED;

@@ -19,6 +19,7 @@
 #include <algorithm>
 
 #include "internal.h"
+#include "sm100_ptx.cuh"
 
 namespace {
 
@@ -46,83 +47,8 @@ struct DmParams {
     uint32_t psi_bytes, tile_bytes, stage_bytes;
 };
 
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
-{
-    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" ::"r"(smem_u32(bar)),
-                 "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "DM_WAIT:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-        "@p bra DM_DONE;\n\t"
-        "bra DM_WAIT;\n\t"
-        "DM_DONE:\n\t"
-        "}" ::"r"(smem_u32(bar)),
-        "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity)
-{
-    uint32_t ok;
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t"
-        "}"
-        : "=r"(ok)
-        : "r"(smem_u32(bar)), "r"(parity)
-        : "memory");
-    return ok != 0;
-}
-__device__ __forceinline__ double lds1(uint32_t addr)
-{
-    double v;
-    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
-    return v;
-}
-__device__ __forceinline__ double2 lds2(uint32_t addr)
-{
-    double2 v;
-    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
-    return v;
-}
-__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap *tmap, uint64_t *bar, int x, int y, int z, int c)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(
-            dst),
-        "l"(tmap), "r"(x), "r"(y), "r"(z), "r"(c), "r"(smem_u32(bar))
-        : "memory");
-}
-__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *tmap, uint64_t *bar, int x, int y, int z)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
-            dst),
-        "l"(tmap), "r"(x), "r"(y), "r"(z), "r"(smem_u32(bar))
-        : "memory");
-}
-__device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b)
-{
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-                 : "+d"(c0), "+d"(c1)
-                 : "d"(a), "d"(b));
-}
+using namespace sm100;
+
 
 template <bool HAS_PREV, int TYB, int MINB>
 __global__ void __launch_bounds__(MINB == 1 ? 13 * 32 : 7 * 32, MINB)
@@ -142,7 +68,7 @@ stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
             mbar_init(&bar_full[s], 1);
             mbar_init(&bar_empty[s], (uint32_t)P.nwarps);
         }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_fence_init();
     }
     __syncthreads();
 
@@ -161,9 +87,9 @@ stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
     if (tid < 32) {
         // ================================ producer warp (one lane) =======================================
         if (tid != 0) return;
-        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_x8) : "memory");
-        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_v) : "memory");
-        if (HAS_PREV) asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_p) : "memory");
+        prefetch_tmap(&tmap_x8);
+        prefetch_tmap(&tmap_v);
+        if (HAS_PREV) prefetch_tmap(&tmap_p);
         const uint32_t row_bytes = (uint32_t)(W * 8);
         const uint32_t tile_tx = (uint32_t)(TY * W * 8);
         // TYB + 2 boxes of 8 rows (128-byte aligned destinations): rows y0-8 .. y0-1 (6 used), the tile, y0+TY ..
@@ -293,24 +219,11 @@ stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
     }
 }
 
-typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
-                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
 // (x, y, z[, column]) tensor map over an N_d x ncols column-major block; box = bx x by x 1 [x 1]
 bool encode_map(const sparc_gpu_ctx *ctx, CUtensorMap *tm, const void *base, int rank, int64_t ncols, int64_t ld, int bx,
                 int by)
 {
-    const int nx = ctx->n[0], ny = ctx->n[1], nz = ctx->n[2];
-    const cuuint64_t gdim[4] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nz, (cuuint64_t)std::max<int64_t>(ncols, 1)};
-    const cuuint64_t gstr[3] = {(cuuint64_t)nx * 8, (cuuint64_t)nx * ny * 8, (cuuint64_t)ld * 8};
-    const cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, 1, 1};
-    const cuuint32_t estr[4] = {1, 1, 1, 1};
-    CUresult cr = ((EncodeTiledFn)ctx->fn_encode_tiled)(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, (cuuint32_t)rank, (void *)base,
-                                                        gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                                        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                                                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    return cr == CUDA_SUCCESS;
+    return encode_grid_map(ctx->fn_encode_tiled, tm, base, ctx->n, rank, ncols, ld, bx, by);
 }
 
 // smallest pitch >= need with pitch mod 16 in {4, 12}: 8 rows x 4 consecutive doubles then tile all 32 banks
@@ -364,16 +277,17 @@ int launch_stencil_dmma(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double
     P.tile_bytes = (uint32_t)(TY * P.W * 8);
     P.stage_bytes = P.psi_bytes + 2 * P.tile_bytes;
     const int threads = (P.nwarps + 1) * 32;
-    // up to 6 consumer warps: two CTAs per SM (128 registers; a third would need <= 80 and spills the z-sums);
-    // more: one CTA of up to 12 consumer warps
-    const bool small = P.nwarps <= 6;
+    // one 8-row block and up to 6 consumer warps: two CTAs per SM (128 registers; a third would need <= 80 and spills the
+    // z-sums); otherwise one CTA of up to 12 consumer warps.  The kernel's TYB must be the one the parameters (boxes per
+    // stage, y tiles, warps) were built for, so it is chosen from tyb first.
+    const bool small = tyb == 1 && P.nwarps <= 6;
     typedef void (*Kern)(const CUtensorMap, const CUtensorMap, const CUtensorMap, const DmParams);
-    Kern kern = small ? (has_prev ? (Kern)stencil_dmma_kernel<true, 1, 2> : (Kern)stencil_dmma_kernel<false, 1, 2>)
-                : tyb == 2 ? (has_prev ? (Kern)stencil_dmma_kernel<true, 2, 1> : (Kern)stencil_dmma_kernel<false, 2, 1>)
-                           : (has_prev ? (Kern)stencil_dmma_kernel<true, 1, 1> : (Kern)stencil_dmma_kernel<false, 1, 1>);
+    Kern kern = tyb == 2 ? (has_prev ? (Kern)stencil_dmma_kernel<true, 2, 1> : (Kern)stencil_dmma_kernel<false, 2, 1>)
+                : small  ? (has_prev ? (Kern)stencil_dmma_kernel<true, 1, 2> : (Kern)stencil_dmma_kernel<false, 1, 2>)
+                         : (has_prev ? (Kern)stencil_dmma_kernel<true, 1, 1> : (Kern)stencil_dmma_kernel<false, 1, 1>);
     // ring depth: as deep as shared memory allows (one or two CTAs per SM by registers); the kernel waits on TMA data
     // more than on anything else
-    const int ctas = (P.nwarps <= 6 && tyb == 1) ? 2 : 1;
+    const int ctas = small ? 2 : 1;
     int nstage = (int)std::min<int64_t>(ctx->opt_stencil_stages > 0 ? ctx->opt_stencil_stages : 6,
                                         (227 * 1024 / ctas - 2048) / P.stage_bytes);
     nstage = std::min(nstage, MAX_STAGES);

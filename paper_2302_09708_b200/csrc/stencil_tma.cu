@@ -22,6 +22,7 @@
 #include <algorithm>
 
 #include "internal.h"
+#include "sm100_ptx.cuh"
 
 namespace {
 
@@ -50,72 +51,8 @@ struct TmaParams {
     uint32_t psi_bytes, tile_bytes, stage_bytes;   // input plane, Veff / Prev tile, whole stage (128-B multiples)
 };
 
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+using namespace sm100;
 
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
-{
-    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" ::"r"(smem_u32(bar)),
-                 "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "WAIT_LOOP:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-        "@p bra WAIT_DONE;\n\t"
-        "bra WAIT_LOOP;\n\t"
-        "WAIT_DONE:\n\t"
-        "}" ::"r"(smem_u32(bar)),
-        "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity)
-{
-    uint32_t ok;
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t"
-        "}"
-        : "=r"(ok)
-        : "r"(smem_u32(bar)), "r"(parity)
-        : "memory");
-    return ok != 0;
-}
-__device__ __forceinline__ double2 lds2(uint32_t addr)
-{
-    double2 v;
-    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
-    return v;
-}
-__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap *tmap, uint64_t *bar, int x, int y, int z, int c)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(
-            dst),
-        "l"(tmap), "r"(x), "r"(y), "r"(z), "r"(c), "r"(smem_u32(bar))
-        : "memory");
-}
-__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *tmap, uint64_t *bar, int x, int y, int z)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
-            dst),
-        "l"(tmap), "r"(x), "r"(y), "r"(z), "r"(smem_u32(bar))
-        : "memory");
-}
 
 // AY: rows per consumer thread (2: 4 points / 168 registers, 1: 2 points / ~100 registers, twice the warps);
 // CW, CNX: compile-time smem pitches (doubles) of the input plane and of the Veff / Prev tiles, 0 = run time (P.W, P.nx).
@@ -137,7 +74,7 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_cons
             mbar_init(&bar_full[s], 1);
             mbar_init(&bar_empty[s], (uint32_t)n_cwarps);
         }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_fence_init();
     }
     __syncthreads();
 
@@ -158,9 +95,9 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_cons
     if (tid < 32) {
         // ================================ producer warp (one lane) =======================================
         if (tid != 0) return;
-        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_x) : "memory");
-        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_v) : "memory");
-        if (HAS_PREV) asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_p) : "memory");
+        prefetch_tmap(&tmap_x);
+        prefetch_tmap(&tmap_v);
+        if (HAS_PREV) prefetch_tmap(&tmap_p);
         const int nboxes = (P.TY + 2 * R) / BOX_ROWS;
         const uint32_t box_bytes = (uint32_t)(BOX_ROWS * W * 8);
         const uint32_t tile_tx = (uint32_t)(P.TY * NX * 8);
@@ -331,7 +268,7 @@ stencil_tma_kernel(const __grid_constant__ CUtensorMap tmap_x, const __grid_cons
     }
 }
 
-struct TileChoice { int AY, TY, threads, ctas_per_sm, nstage, W, variant; uint32_t psi_bytes, tile_bytes, stage_bytes; size_t smem; };
+typedef StencilTileChoice TileChoice;
 
 constexpr int SMEM_PER_SM = 227 * 1024;
 
@@ -362,7 +299,7 @@ StencilKernel pick_kernel(int ay, int variant, bool has_prev)
 // Tile rows TY: a multiple of 6 (TMA box rows) and of AY dividing ny.  Preference: the tallest tile whose CTA still
 // fits at least twice on an SM (the kernels are register-limited), else the smallest valid tile.  The ring depth is
 // whatever the per-CTA share of shared memory allows.
-bool choose_tile(const sparc_gpu_ctx *ctx, TileChoice *tc)
+bool compute_tile(const sparc_gpu_ctx *ctx, TileChoice *tc)
 {
     const int nx = ctx->n[0], ny = ctx->n[1];
     const int ntx = nx / 2;
@@ -423,26 +360,26 @@ bool choose_tile(const sparc_gpu_ctx *ctx, TileChoice *tc)
     return false;
 }
 
-bool a16(const void *p) { return ((uintptr_t)p & 15) == 0; }
+// the choice depends only on the grid, the boundary flags and the stencil_* options: computed once per context
+// (sparc_gpu_set_option invalidates it), so a degree step costs no occupancy queries
+bool choose_tile(const sparc_gpu_ctx *ctx, TileChoice *tc)
+{
+    if (ctx->tma_choice.valid == 0) {
+        TileChoice t;
+        t.valid = compute_tile(ctx, &t) ? 1 : -1;
+        ctx->tma_choice = t;
+    }
+    *tc = ctx->tma_choice;
+    return tc->valid == 1;
+}
 
-typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
-                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+bool a16(const void *p) { return ((uintptr_t)p & 15) == 0; }
 
 // (x, y, z[, column]) tensor map over an N_d x ncols column-major block; box = bx x by x 1 [x 1]
 bool encode_map(const sparc_gpu_ctx *ctx, CUtensorMap *tm, const void *base, int rank, int64_t ncols, int64_t ld, int bx,
                 int by)
 {
-    const int nx = ctx->n[0], ny = ctx->n[1], nz = ctx->n[2];
-    const cuuint64_t gdim[4] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nz, (cuuint64_t)std::max<int64_t>(ncols, 1)};
-    const cuuint64_t gstr[3] = {(cuuint64_t)nx * 8, (cuuint64_t)nx * ny * 8, (cuuint64_t)ld * 8};
-    const cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, 1, 1};
-    const cuuint32_t estr[4] = {1, 1, 1, 1};
-    CUresult cr = ((EncodeTiledFn)ctx->fn_encode_tiled)(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, (cuuint32_t)rank, (void *)base,
-                                                        gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                                        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                                                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    return cr == CUDA_SUCCESS;
+    return encode_grid_map(ctx->fn_encode_tiled, tm, base, ctx->n, rank, ncols, ld, bx, by);
 }
 
 }  // namespace

@@ -52,6 +52,7 @@ def sample_columns(ns, block, n_random, rng):
         cols.add(j0)
         cols.add(min(j0 + block, ns) - 1)
     cols.update(int(c) for c in rng.choice(ns, size=min(n_random, ns), replace=False))
+    cols.update(int(c) for c in rng.choice(min(block, ns), size=min(4, block, ns), replace=False))   # inside the first block
     return sorted(cols)
 
 
@@ -86,9 +87,18 @@ def fullsize_parity(torch, api, cfg, n_random_cols, n_gram, n_random_rows, check
     assert np.array_equal(api.colmajor_to_numpy(Psi[idx]), X), "device fill != host generator"
     norm2 = float(torch.linalg.vector_norm(Psi)) ** 2
 
-    # ---- H*Psi on the sampled columns -----------------------------------------------------------------------
-    Yg = g.hamiltonian_apply(Psi[idx].contiguous())
+    # ---- H*Psi: the whole first column block in ONE call (bench.py's launch configuration: col_block columns per
+    # kernel launch), compared on the sampled columns that fall inside it; then the remaining sampled columns gathered
     HX = H.apply(X)
+    nb = min(col_block, ns)
+    Yblk = g.hamiltonian_apply(Psi[:nb])
+    inblk = [k for k, cidx in enumerate(cols) if cidx < nb]
+    assert len(inblk) >= 2
+    e = col_err(api.colmajor_to_numpy(Yblk[torch.tensor([cols[k] for k in inblk], device=dev)]), HX[:, inblk])
+    print(f"[parity] cfg{cfg} H*Psi, {nb}-column launch, {len(inblk)} sampled columns of it: {e:.3e}")
+    assert e <= TOL_COL and e <= TIGHT
+    del Yblk
+    Yg = g.hamiltonian_apply(Psi[idx].contiguous())
     e = col_err(api.colmajor_to_numpy(Yg), HX)
     print(f"[parity] cfg{cfg} H*Psi, {len(cols)} sampled columns: {e:.3e}")
     assert e <= TOL_COL and e <= TIGHT

@@ -167,20 +167,24 @@ def test_brick_shapes_and_classes(torch, api, nx, projs):
     g.set_option("nonlocal_mode", 3)
     X = wl.psi_columns(range(wl.ns))
     H = orc.Hamiltonian(wl)
-    for tile_io in (1, 0):          # 1: direct global loads / stores of the tile, 0: staged by TMA (default)
-        g.set_option("nlb_tma", tile_io)
+    # persistent kernel (the default when every brick's chi blocks fit its store); general kernel with all blocks
+    # resident; general kernel with forced load rounds
+    for kern, cap in ((2, 0), (1, 0), (1, 16)):
+        g.set_option("nlb_kernel", kern)
+        g.set_option("nlb_cap", cap)
         Yg = g.hamiltonian_apply(api.colmajor_from_numpy(X))
-        check_col(api.colmajor_to_numpy(Yg), H.apply(X), f"brick nx={nx} P={projs} H*Psi tile_io={tile_io}")
-    for m, cb in ((1, 0), (4, 5)):
-        Pg = api.colmajor_from_numpy(X)
-        g.chebyshev_filter(Pg, m, wl.a, wl.b, wl.a0, col_block=cb)
-        check_col(api.colmajor_to_numpy(Pg), H.chebyshev_filter(X, m, wl.a, wl.b, wl.a0), f"brick nx={nx} filter m={m}")
+        check_col(api.colmajor_to_numpy(Yg), H.apply(X), f"brick nx={nx} P={projs} H*Psi kernel={kern} cap={cap}")
+        for m, cb in ((1, 0), (4, 5)):
+            Pg = api.colmajor_from_numpy(X)
+            g.chebyshev_filter(Pg, m, wl.a, wl.b, wl.a0, col_block=cb)
+            check_col(api.colmajor_to_numpy(Pg), H.chebyshev_filter(X, m, wl.a, wl.b, wl.a0),
+                      f"brick nx={nx} filter m={m} kernel={kern} cap={cap}")
     g.close()
 
 
 def test_brick_many_atoms_per_brick(torch, api):
-    """More (brick, atom) jobs per brick than the kernel keeps in flight (16 slots, 32-job descriptor batches), so
-    that the producer warp wraps its slots and its byte ring; 70 columns = one full and one ragged column group."""
+    """Many (brick, atom) jobs per brick (24 overlapping atoms), with the block store capped so that a brick needs
+    several load rounds in both phases; 70 columns = one full and one ragged column group."""
     rng = np.random.default_rng(3)
     pos = rng.uniform(0.0, 4.8, size=(24, 3))
     wl = wlmod.make_custom("dense_atoms", (16, 16, 16), (0.3, 0.3, 0.3), (0, 0, 0), 70, 3, pos, [9] * 24, 2.0, seed=8)
@@ -189,11 +193,162 @@ def test_brick_many_atoms_per_brick(torch, api):
     g.set_option("nonlocal_mode", 3)
     X = wl.psi_columns(range(wl.ns))
     H = orc.Hamiltonian(wl)
+    HX, F3 = H.apply(X), H.chebyshev_filter(X, 3, wl.a, wl.b, wl.a0)
+    for cap in (0, 40, 16):
+        g.set_option("nlb_cap", cap)
+        Yg = g.hamiltonian_apply(api.colmajor_from_numpy(X))
+        check_col(api.colmajor_to_numpy(Yg), HX, f"dense atoms H*Psi cap={cap}")
+        Pg = api.colmajor_from_numpy(X)
+        g.chebyshev_filter(Pg, 3, wl.a, wl.b, wl.a0)
+        check_col(api.colmajor_to_numpy(Pg), F3, f"dense atoms filter m=3 cap={cap}")
+    g.close()
+
+
+def test_brick_more_jobs_than_barriers(torch, api):
+    """More than 32 atoms meeting one brick (the kernel has 32 job barriers per load round), negative and zero gamma."""
+    rng = np.random.default_rng(5)
+    pos = 2.4 + rng.uniform(-0.5, 0.5, size=(40, 3))
+    gam = rng.uniform(-1.0, 1.0, size=40 * 4)
+    gam[::7] = 0.0
+    wl = wlmod.make_custom("jobs40", (16, 16, 16), (0.3, 0.3, 0.3), (0, 1, 0), 9, 3, pos, [4] * 40, 1.5, seed=9, gamma=gam)
+    g = api.SparcGpu(wl)
+    assert g.get_info("nl_brick") == 1
+    g.set_option("nonlocal_mode", 3)
+    X = wl.psi_columns(range(wl.ns))
+    H = orc.Hamiltonian(wl)
     Yg = g.hamiltonian_apply(api.colmajor_from_numpy(X))
-    check_col(api.colmajor_to_numpy(Yg), H.apply(X), "dense atoms H*Psi")
+    check_col(api.colmajor_to_numpy(Yg), H.apply(X), "40 atoms per brick H*Psi")
     Pg = api.colmajor_from_numpy(X)
     g.chebyshev_filter(Pg, 3, wl.a, wl.b, wl.a0)
-    check_col(api.colmajor_to_numpy(Pg), H.chebyshev_filter(X, 3, wl.a, wl.b, wl.a0), "dense atoms filter m=3")
+    check_col(api.colmajor_to_numpy(Pg), H.chebyshev_filter(X, 3, wl.a, wl.b, wl.a0), "40 atoms per brick filter")
+    g.close()
+
+
+@pytest.mark.parametrize("bc", [(0, 0, 0), (1, 1, 1), (0, 1, 0)])
+@pytest.mark.parametrize("knob", [("stencil_ay", 1, 2), ("stencil_ay", 2, 2), ("stencil_ty", 16, 3), ("stencil_stages", 2, 3),
+                                  ("stencil_zchunks", 3, 2)])
+def test_stencil_tile_knobs(torch, api, knob, bc):
+    """Every compiled stencil variant reachable through set_option runs against the oracle: AY = 1 (320 threads, two CTAs
+    per SM) and AY = 2 of the TMA kernel, the TYB = 2 (16-row) tile of the hybrid kernel on a narrow (2 * nxb <= 6) and on a
+    wide grid, a two-stage ring, forced z chunks."""
+    key, val, path = knob
+    pos = np.array([[1.0, 2.0, 3.0], [3.5, 4.0, 0.4]])
+    for n in ((24, 48, 17), (48, 48, 14)):
+        wl = wlmod.make_custom(f"knob_{key}{val}_{n}_{bc}", n, (0.4, 0.45, 0.5), bc, 4, 5, pos, [4, 9], 2.2, seed=29)
+        g = api.SparcGpu(wl)
+        g.set_option("stencil_path", path)
+        g.set_option(key, val)
+        X = wl.psi_columns(range(wl.ns))
+        H = orc.Hamiltonian(wl)
+        Yg = g.hamiltonian_apply(api.colmajor_from_numpy(X))
+        check_col(api.colmajor_to_numpy(Yg), H.apply(X), f"{wl.name} H*Psi")
+        assert g.get_info("stencil_path_last") == path
+        Pg = api.colmajor_from_numpy(X)
+        g.chebyshev_filter(Pg, wl.degree, wl.a, wl.b, wl.a0)
+        check_col(api.colmajor_to_numpy(Pg), H.chebyshev_filter(X, wl.degree, wl.a, wl.b, wl.a0), f"{wl.name} filter")
+        g.close()
+
+
+def test_stencil_stage_option_is_validated(torch, api):
+    wl = wlmod.make_workload(0)
+    g = api.SparcGpu(wl)
+    with pytest.raises(api.SparcGpuError) as ei:
+        g.set_option("stencil_stages", 1)          # a one-stage ring is refused up front, not at launch
+    assert ei.value.code == -1
+    g.close()
+
+
+def test_set_veff(torch, api):
+    """sparc_gpu_set_veff (a new effective potential every SCF iteration): create with veff = NULL
+    (zero potential until set), set, compare H*Psi and the filter with the oracle; set a second potential, compare again;
+    on every stencil path (the TMA kernels read Veff through a tensor map of the context's buffer)."""
+    pos = np.array([[1.0, 2.0, 3.0], [5.5, 5.0, 0.4]])
+    base = wlmod.make_custom("veff_a", (24, 24, 16), (0.4, 0.45, 0.5), (0, 0, 1), 6, 5, pos, [9, 4], 2.4, seed=31)
+    other = wlmod.make_custom("veff_b", (24, 24, 16), (0.4, 0.45, 0.5), (0, 0, 1), 6, 5, pos + 0.7, [9, 4], 2.4, seed=32)
+    import copy
+    X = base.psi_columns(range(base.ns))
+    for path in (1, 2, 3):
+        g = api.SparcGpu(base, upload_veff=False)                  # desc.veff = NULL
+        g.set_option("stencil_path", path)
+        zero = copy.copy(base); zero.veff = np.zeros(base.nd)
+        Yg = g.hamiltonian_apply(api.colmajor_from_numpy(X))
+        check_col(api.colmajor_to_numpy(Yg), orc.Hamiltonian(zero).apply(X), f"veff NULL at create, path {path}")
+        for tag, v in (("first", base.veff), ("second", other.veff)):
+            wl = copy.copy(base); wl.veff = np.ascontiguousarray(v)
+            g.set_veff(torch.from_numpy(wl.veff).cuda())
+            H = orc.Hamiltonian(wl)
+            Yg = g.hamiltonian_apply(api.colmajor_from_numpy(X))
+            check_col(api.colmajor_to_numpy(Yg), H.apply(X), f"set_veff {tag}, path {path}: H*Psi")
+            Pg = api.colmajor_from_numpy(X)
+            g.chebyshev_filter(Pg, 4, base.a, base.b, base.a0 - 1.0)
+            check_col(api.colmajor_to_numpy(Pg), H.chebyshev_filter(X, 4, base.a, base.b, base.a0 - 1.0),
+                      f"set_veff {tag}, path {path}: filter")
+        g.close()
+
+
+def test_operators_on_a_non_default_stream(torch, api):
+    """Every operator is asynchronous on the stream it is given (include/sparc_gpu.h): run filter, project, rotate and
+    H*Psi on a side stream while a second stream keeps the device busy, with the inputs produced on the side stream just
+    before; results must match the oracle and nothing may have been enqueued on the default stream."""
+    wl = wlmod.make_workload(0)
+    g = api.SparcGpu(wl)
+    H = orc.Hamiltonian(wl)
+    X = wl.psi()
+    O = H.chebyshev_filter(X, wl.degree, wl.a, wl.b, wl.a0)
+    side, noise = torch.cuda.Stream(), torch.cuda.Stream()
+    junk = torch.empty(64 << 20, dtype=torch.float64, device="cuda")
+    host_X = torch.from_numpy(np.ascontiguousarray(X.T)).pin_memory()
+    Qn = wl.q_matrix()
+    host_Q = torch.from_numpy(np.ascontiguousarray(Qn.T)).pin_memory()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(noise):
+        for _ in range(20):
+            junk.mul_(1.0000001)
+    with torch.cuda.stream(side):
+        Pg = torch.empty((wl.ns, wl.nd), dtype=torch.float64, device="cuda")
+        Pg.copy_(host_X, non_blocking=True)                       # input produced on the side stream
+        Qg = torch.empty((wl.ns, wl.ns), dtype=torch.float64, device="cuda")
+        Qg.copy_(host_Q, non_blocking=True)
+        Yg = g.hamiltonian_apply(Pg)
+        g.chebyshev_filter(Pg, wl.degree, wl.a, wl.b, wl.a0)
+        Fg = Pg.clone()
+        Hs, Ms = g.project(Pg)
+        g.rotate(Pg, Qg)
+    side.synchronize()
+    check_col(api.colmajor_to_numpy(Yg), H.apply(X), "side stream H*Psi")
+    check_col(api.colmajor_to_numpy(Fg), O, "side stream filter")
+    Hs_o, Ms_o = H.project(O)
+    check_fro(api.colmajor_to_numpy(Hs), Hs_o, "side stream Hs")
+    check_fro(api.colmajor_to_numpy(Ms), Ms_o, "side stream Ms")
+    check_fro(api.colmajor_to_numpy(Pg), orc.rotate(O, Qn), "side stream Psi*Q")
+    torch.cuda.synchronize()
+    g.close()
+
+
+def test_workspace_too_small_is_an_error_code(torch, api):
+    """A declared workspace size turns a short buffer into WORKSPACE_TOO_SMALL (-5) instead of an overrun."""
+    import ctypes as C
+    wl = wlmod.make_workload(0)
+    g = api.SparcGpu(wl)
+    lib = g.lib
+    Pg = api.colmajor_from_numpy(wl.psi())
+    need = g.workspace_bytes(api.OP_CHEBYSHEV_FILTER, wl.ns, 0)
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    st = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    args = (g._ctx, C.c_void_p(Pg.data_ptr()), wl.nd, wl.ns, 2, wl.a, wl.b, wl.a0, 0, C.c_void_p(ws.data_ptr()), st)
+    assert lib.sparc_gpu_set_workspace_size(g._ctx, need - 1) == 0
+    before = Pg.clone()
+    assert lib.sparc_gpu_chebyshev_filter(*args) == -5
+    assert torch.equal(Pg, before)                                 # nothing ran
+    Hs = torch.empty((wl.ns, wl.ns), dtype=torch.float64, device="cuda")
+    assert lib.sparc_gpu_project(g._ctx, C.c_void_p(Pg.data_ptr()), wl.nd, wl.ns, C.c_void_p(Hs.data_ptr()),
+                                 C.c_void_p(Hs.data_ptr()), 0, C.c_void_p(ws.data_ptr()), st) == -5
+    assert lib.sparc_gpu_rotate(g._ctx, C.c_void_p(Pg.data_ptr()), wl.nd, wl.ns, C.c_void_p(Hs.data_ptr()), 0,
+                                C.c_void_p(ws.data_ptr()), st) in (0, -5)
+    assert lib.sparc_gpu_set_workspace_size(g._ctx, -1) == -1
+    assert lib.sparc_gpu_set_workspace_size(g._ctx, need) == 0
+    assert lib.sparc_gpu_chebyshev_filter(*args) == 0
+    torch.cuda.synchronize()
     g.close()
 
 
