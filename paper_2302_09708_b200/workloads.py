@@ -19,7 +19,8 @@ fill kernel (``sparc_gpu_fill_uniform``) so that an 82 GB Psi never crosses PCIe
 two implementations are independent restatements of the recipe documented here.
 
 Streams: 1 = Psi, 2 = Veff noise, 3 = atom positions / jitter, 4 = Veff centres,
-5 = gamma, 6 = Q (Gaussian matrix), 7 = Veff smooth-noise parameters.
+5 = gamma, 6 = Q (Gaussian matrix), 7 = Veff smooth-noise parameters, 8 = imaginary part of a complex Psi,
+9 = occupations.
 """
 from __future__ import annotations
 
@@ -36,6 +37,8 @@ STREAM_VEFF_CENTRES = 4
 STREAM_GAMMA = 5
 STREAM_Q = 6
 STREAM_VEFF_SMOOTH = 7
+STREAM_PSI_IMAG = 8
+STREAM_OCC = 9
 
 _M64 = (1 << 64) - 1
 _GOLDEN = 0x9E3779B97F4A7C15
@@ -104,6 +107,7 @@ class Workload:
     col_block: int = 0                 # filter column block (0 = library chooses)
     row_panel: int = 0                 # rotation row panel (0 = library chooses)
     notes: str = ""
+    supp_shift: Optional[np.ndarray] = None   # [supp_total, 3] int8: cells each support row was folded by (k-point phases)
 
     @property
     def nd(self) -> int:
@@ -147,6 +151,24 @@ class Workload:
             out[:, j] = 2.0 * counter_uniform(self.seed, STREAM_PSI, r + np.uint64(nd * j)) - 1.0
         return out
 
+    def psi_columns_complex(self, cols: Sequence[int]) -> np.ndarray:
+        """Complex columns for the k-point variant: real part as psi_columns, imaginary part from STREAM_PSI_IMAG."""
+        nd = self.nd
+        out = np.empty((nd, len(cols)), dtype=np.complex128, order="F")
+        base = np.arange(nd, dtype=np.uint64)
+        for k, j in enumerate(cols):
+            idx = base + np.uint64(nd * int(j))
+            out[:, k] = (2.0 * counter_uniform(self.seed, STREAM_PSI, idx) - 1.0) + 1j * (
+                2.0 * counter_uniform(self.seed, STREAM_PSI_IMAG, idx) - 1.0)
+        return out
+
+    def occupations(self) -> np.ndarray:
+        """Synthetic occupation numbers g_n in [0, 2] (spin-degenerate), decreasing with the orbital index: inputs of
+        the nonlocal-force contraction."""
+        u = counter_uniform_range(self.seed, STREAM_OCC, 0, self.ns)
+        x = (np.arange(self.ns) + u) / max(self.ns, 1)
+        return 2.0 / (1.0 + np.exp(12.0 * (x - 0.85)))
+
     def q_matrix(self) -> np.ndarray:
         """Haar-random orthogonal Q (ns x ns, Fortran order): Gaussian matrix -> QR -> sign fix."""
         ns = self.ns
@@ -175,12 +197,14 @@ def _axis_offsets(pos: float, h: float, n: int, bc: int, rc: float):
     d = k * h - pos                              # displacement grid point - atom
     if bc == 0:
         idx = np.mod(k, n)
+        wrap = np.floor_divide(k, n)             # cells the true support point lies beyond the cell (image shift)
     else:
         keep = (k >= 0) & (k < n)
         k, d = k[keep], d[keep]
         idx = k
+        wrap = np.zeros_like(k)
     keep = np.abs(d) <= rc + 1e-12
-    return idx[keep].astype(np.int64), d[keep]
+    return idx[keep].astype(np.int64), d[keep], wrap[keep].astype(np.int8)
 
 
 def real_harmonics(dx, dy, dz, r, n_proj: int) -> np.ndarray:
@@ -219,20 +243,22 @@ def build_projectors(n, h, bc, atom_pos, n_proj, rc, width: float = 1.0):
     nx, ny, nz = n
     supp_ptr = [0]
     chi_ptr = [0]
-    idx_all, chi_all = [], []
+    idx_all, chi_all, shift_all = [], [], []
     for J in range(atom_pos.shape[0]):
         P = int(n_proj[J])
-        ix, dx = _axis_offsets(atom_pos[J, 0], h[0], nx, bc[0], rc)
-        iy, dy = _axis_offsets(atom_pos[J, 1], h[1], ny, bc[1], rc)
-        iz, dz = _axis_offsets(atom_pos[J, 2], h[2], nz, bc[2], rc)
+        ix, dx, wx = _axis_offsets(atom_pos[J, 0], h[0], nx, bc[0], rc)
+        iy, dy, wy = _axis_offsets(atom_pos[J, 1], h[1], ny, bc[1], rc)
+        iz, dz, wz = _axis_offsets(atom_pos[J, 2], h[2], nz, bc[2], rc)
         DX, DY, DZ = np.meshgrid(dx, dy, dz, indexing="ij")
         IX, IY, IZ = np.meshgrid(ix, iy, iz, indexing="ij")
+        WX, WY, WZ = np.meshgrid(wx, wy, wz, indexing="ij")
         r = np.sqrt(DX * DX + DY * DY + DZ * DZ).ravel()
         keep = r <= rc
         lin = (IX + nx * (IY + ny * IZ)).ravel()[keep]
         dxk, dyk, dzk, rk = DX.ravel()[keep], DY.ravel()[keep], DZ.ravel()[keep], r[keep]
         order = np.argsort(lin, kind="stable")
         lin, dxk, dyk, dzk, rk = lin[order], dxk[order], dyk[order], dzk[order], rk[order]
+        shift_all.append(np.stack([WX.ravel()[keep][order], WY.ravel()[keep][order], WZ.ravel()[keep][order]], axis=1))
         if lin.size > 1 and np.any(np.diff(lin) == 0):
             raise ValueError("atom support wraps onto itself (need 2*rc < L on periodic axes)")
         radial = np.exp(-(rk * rk) / (2.0 * width * width))
@@ -243,8 +269,9 @@ def build_projectors(n, h, bc, atom_pos, n_proj, rc, width: float = 1.0):
         chi_ptr.append(chi_ptr[-1] + lin.size * P)
     supp_idx = np.concatenate(idx_all) if idx_all else np.zeros(0, np.int32)
     chi = np.concatenate(chi_all) if chi_all else np.zeros(0, np.float64)
+    shift = np.concatenate(shift_all).astype(np.int8) if shift_all else np.zeros((0, 3), np.int8)
     return (np.asarray(supp_ptr, np.int64), supp_idx.astype(np.int32),
-            np.asarray(chi_ptr, np.int64), chi.astype(np.float64))
+            np.asarray(chi_ptr, np.int64), chi.astype(np.float64), shift)
 
 
 def _min_image(d, L, periodic: bool):
@@ -372,11 +399,15 @@ CONFIG_TABLE = {
             atoms=512, P=9, rc=3.5),
     4: dict(name="cfg4_metallic_96x96x144", n=(96, 96, 144), h=0.3, bc=(0, 0, 0), ns=7680, degree=24,
             atoms=1000, P=9, rc=3.5, col_block=1024),
+    # sixth workload: the paper's finer-mesh regime, h = 0.22 bohr and Chebyshev degree 33
+    # (PAPER.md:182), on a grid one GPU holds
+    5: dict(name="cfg5_fine_mesh_128", n=(128, 128, 128), h=0.22, bc=(0, 0, 0), ns=2048, degree=33,
+            atoms=216, P=9, rc=3.5, col_block=1024),
 }
 
 
 def make_workload(config: int, ns: Optional[int] = None) -> Workload:
-    """Workload `config` in 0..4 (BASELINE.json:configs); seed = config number.
+    """Workload `config` in 0..4 (BASELINE.json:configs) or 5 (the finer-mesh, degree-33 regime); seed = config number.
 
     `ns` overrides the orbital count (used by bounded CPU samples; Psi columns are
     position-independent streams, so a prefix of columns is the same data)."""
@@ -402,6 +433,9 @@ def make_workload(config: int, ns: Optional[int] = None) -> Workload:
     elif config == 4:
         pos = _lattice_positions(seed, (5, 5, 10), _FCC, (0, 0, 0), L, 0.3)
         centres = pos
+    elif config == 5:
+        pos = _lattice_positions(seed, (6, 6, 6), _SC, (0, 0, 0), L, 0.3)
+        centres = pos
     else:
         raise KeyError(config)
     # wrap periodic coordinates into the cell (positions are inputs; wrapping is cosmetic)
@@ -409,13 +443,13 @@ def make_workload(config: int, ns: Optional[int] = None) -> Workload:
         if bc[ax] == 0:
             pos[:, ax] = np.mod(pos[:, ax], L[ax])
     n_proj = np.full(c["atoms"], c["P"], dtype=np.int32)
-    supp_ptr, supp_idx, chi_ptr, chi = build_projectors(n, h, bc, pos, n_proj, c["rc"], 1.0)
+    supp_ptr, supp_idx, chi_ptr, chi, supp_shift = build_projectors(n, h, bc, pos, n_proj, c["rc"], 1.0)
     gamma = 2.0 * counter_uniform_range(seed, STREAM_GAMMA, 0, int(n_proj.sum())) - 1.0
     veff = gaussian_wells(n, h, bc, centres, -2.0, 1.5)
     nd = n[0] * n[1] * n[2]
     if config == 0:
         veff = veff + 0.05 * (2.0 * counter_uniform_range(seed, STREAM_VEFF_NOISE, 0, nd) - 1.0)
-    elif config in (1, 3, 4):
+    elif config in (1, 3, 4, 5):
         veff = veff + _smooth_noise(seed, n, h)
     elif config == 2:
         z = (np.arange(n[2]) * h[2])[:, None, None] + np.zeros((1, n[1], n[0]))
@@ -425,7 +459,7 @@ def make_workload(config: int, ns: Optional[int] = None) -> Workload:
                     ns=int(ns if ns is not None else c["ns"]), degree=c["degree"], atom_pos=pos,
                     n_proj=n_proj, rc=c["rc"], supp_ptr=supp_ptr, supp_idx=supp_idx, chi_ptr=chi_ptr,
                     chi=chi, gamma=gamma, veff=np.ascontiguousarray(veff), a0=a0, a=a, b=b,
-                    col_block=c.get("col_block", 0))
+                    col_block=c.get("col_block", 0), supp_shift=supp_shift)
 
 
 def make_custom(name, n, h, bc, ns, degree, atom_pos, n_proj, rc, seed=1234, fd_order=12,
@@ -436,7 +470,7 @@ def make_custom(name, n, h, bc, ns, degree, atom_pos, n_proj, rc, seed=1234, fd_
     bc = tuple(int(v) for v in bc)
     atom_pos = np.asarray(atom_pos, dtype=np.float64).reshape(-1, 3)
     n_proj = np.asarray(n_proj, dtype=np.int32).reshape(-1)
-    supp_ptr, supp_idx, chi_ptr, chi = build_projectors(n, h, bc, atom_pos, n_proj, rc, 1.0)
+    supp_ptr, supp_idx, chi_ptr, chi, supp_shift = build_projectors(n, h, bc, atom_pos, n_proj, rc, 1.0)
     if gamma is None:
         gamma = 2.0 * counter_uniform_range(seed, STREAM_GAMMA, 0, int(n_proj.sum())) - 1.0
     gamma = np.asarray(gamma, dtype=np.float64)
@@ -455,4 +489,4 @@ def make_custom(name, n, h, bc, ns, degree, atom_pos, n_proj, rc, seed=1234, fd_
     return Workload(name=name, seed=seed, n=n, h=h, bc=bc, fd_order=fd_order, ns=ns, degree=degree,
                     atom_pos=atom_pos, n_proj=n_proj, rc=rc, supp_ptr=supp_ptr, supp_idx=supp_idx,
                     chi_ptr=chi_ptr, chi=chi, gamma=gamma, veff=np.ascontiguousarray(veff),
-                    a0=a0, a=a, b=b)
+                    a0=a0, a=a, b=b, supp_shift=supp_shift)
