@@ -64,7 +64,10 @@ typedef enum {
     SPARC_GPU_OP_HAMILTONIAN_APPLY = 0,
     SPARC_GPU_OP_CHEBYSHEV_FILTER = 1,
     SPARC_GPU_OP_PROJECT = 2,
-    SPARC_GPU_OP_ROTATE = 3
+    SPARC_GPU_OP_ROTATE = 3,
+    SPARC_GPU_OP_GRADIENT_PROJECT = 4,
+    SPARC_GPU_OP_NONLOCAL_FORCE = 5,
+    SPARC_GPU_OP_EIGENSOLVE = 6
 } sparc_gpu_op;
 
 /* Problem description (all pointers HOST, copied at create).  PAPER.md:118 "The matrix X, effective
@@ -129,6 +132,61 @@ int sparc_gpu_project(sparc_gpu_ctx *ctx, const double *Psi_dev, int64_t ld, int
  * workspace.  The result does not depend on row_panel (R19). */
 int sparc_gpu_rotate(sparc_gpu_ctx *ctx, double *Psi_dev, int64_t ld, int64_t ns, const double *Q_dev,
                      int64_t row_panel, void *ws_dev, void *stream);
+
+/* ---- gradient stencil and projector contraction for the nonlocal force ----------------
+ * PAPER.md:110 "the application of the gradient operator on the Kohn-Sham orbitals" and "nonlocal projector
+ * multiplications" are the two kernels of the nonlocal Hellmann-Feynman force. */
+
+/* Y = D_axis X on ncols columns: central finite-difference FIRST derivative of the same order n0 as the Laplacian
+ * (radius n0/2; weights w_p = (-1)^{p+1} (n!)^2 / (p (n-p)! (n+p)!), w_{-p} = -w_p, reading R21), along axis 0 (x), 1 (y)
+ * or 2 (z); periodic axes wrap, neighbours outside a Dirichlet face contribute 0 (R9).  X and Y must not overlap. */
+int sparc_gpu_gradient(sparc_gpu_ctx *ctx, int axis, const double *X_dev, int64_t ldx, double *Y_dev, int64_t ldy,
+                       int64_t ncols, void *stream);
+
+/* W = chi^T X: W[po_J + q, col] = sum_t chi_J[t, q] X[idx_J[t], col], po_J = sum_{I<J} P_I; no Gamma, no volume factor
+ * (R6, R7).  W_dev: n_proj_total x ncols column-major, ld = n_proj_total. */
+int sparc_gpu_nl_project(sparc_gpu_ctx *ctx, const double *X_dev, int64_t ldx, int64_t ncols, double *W_dev, void *stream);
+
+/* W = chi^T (D_axis X), the gradient formed by column blocks in the workspace (op GRADIENT_PROJECT). */
+int sparc_gpu_gradient_project(sparc_gpu_ctx *ctx, int axis, const double *X_dev, int64_t ldx, int64_t ncols,
+                               double *W_dev, int64_t col_block, void *ws_dev, void *stream);
+
+/* Nonlocal Hellmann-Feynman force (reading R22):
+ *   F[J, a] = -2 sum_n occ[n] sum_q gamma_Jq (chi_Jq^T psi_n) (chi_Jq^T D_a psi_n),
+ * occ_dev[ns] = occupation (times spin degeneracy) of each orbital; F_dev: n_atoms x 3 doubles, row-major (F[3 J + a]),
+ * overwritten.  Workspace op NONLOCAL_FORCE.  Bitwise reproducible (fixed reduction order). */
+int sparc_gpu_nonlocal_force(sparc_gpu_ctx *ctx, const double *Psi_dev, int64_t ld, int64_t ns, const double *occ_dev,
+                             double *F_dev, int64_t col_block, void *ws_dev, void *stream);
+
+/* ---- the subspace eigenproblem on the device ---------------------------------------------
+ * Generalized symmetric-definite eigenproblem  Hs Z = Ms Z D  of the subspace step (Algorithm 1
+ * "Subspace diagonalization", 148-154 eq. 9; the paper calls cusolverDnDsygvd).  Hs symmetric, Ms symmetric positive
+ * definite, both n x n column-major (ld = n), read only.  Outputs: D_dev[n] ascending; Z_dev n x n column-major with
+ * Z^T Ms Z = I, unique up to the sign of each column and rotations inside degenerate eigenspaces (reading R23) -- Z is the Q
+ * of sparc_gpu_rotate.  Method: Cholesky Ms = L L^T, A = L^-1 Hs L^-T, one-sided Jacobi on a Cholesky factor of the shifted
+ * A, Rayleigh-quotient eigenvalues, Z = L^-T V (csrc/eig.cu).  Everything is queued on `stream`; convergence is tested on the
+ * device.  info_dev (2 x int32, may be NULL): [0] status 0 ok / 1 Ms not positive definite / 2 not converged, [1] sweeps.
+ * Workspace op EIGENSOLVE with ns = n.  n <= 12800 (a column pair must fit shared memory), else UNSUPPORTED. */
+int sparc_gpu_eigensolve(sparc_gpu_ctx *ctx, int64_t n, const double *Hs_dev, const double *Ms_dev, double *Z_dev,
+                         double *D_dev, int32_t *info_dev, void *ws_dev, void *stream);
+
+/* One whole CheFSI step -- filter, project, rotate -- for a block that lives in HOST memory (what the paper's code does
+ * around every step with cublasSet/GetVector: PAPER.md:118, 128, 138, 146, 158, 166), with the PCIe copies overlapped with
+ * the kernels: columns are uploaded chunk by chunk while earlier chunks are filtered (columns are independent,
+ * PAPER.md:120); Hs and Ms are downloaded when the projection is done; the rotation runs row panel by row panel
+ * and every finished panel is downloaded while the next one is multiplied.
+ *   Psi_in_host, Psi_out_host : N_d x ns column-major, ld_host >= N_d, HOST (pinned memory for full PCIe rate; they may
+ *                               be the same buffer)
+ *   Q_host (in), Hs_host, Ms_host (out) : ns x ns column-major HOST.  Q is the caller's eigenvector matrix; the
+ *                               eigensolve stays outside this call (a caller that needs Hs, Ms first uses
+ *                               sparc_gpu_eigensolve on the device or the separate operator calls)
+ *   Psi_dev  : DEVICE scratch for the block, N_d x ns with ld_dev >= N_d;  mats_dev: DEVICE scratch of 3 ns^2 doubles
+ *   ws_dev   : DEVICE scratch of max(workspace_bytes(CHEBYSHEV_FILTER), workspace_bytes(PROJECT), workspace_bytes(ROTATE))
+ * Work is queued on `stream` and two copy streams owned by the context; the call SYNCHRONISES all three before it returns. */
+int sparc_gpu_chefsi_step_host(sparc_gpu_ctx *ctx, const double *Psi_in_host, double *Psi_out_host, int64_t ld_host,
+                               int64_t ns, int degree, double a, double b, double a0, const double *Q_host,
+                               double *Hs_host, double *Ms_host, double *Psi_dev, int64_t ld_dev, double *mats_dev,
+                               int64_t col_block, int64_t row_panel, void *ws_dev, void *stream);
 
 /* ---- support entry points (not operators of the method) ------------------------------------- */
 

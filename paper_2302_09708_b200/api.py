@@ -21,11 +21,13 @@ _LIB_PATH = os.path.join(_HERE, "libsparc_gpu.so")
 _lib = None
 
 OP_HAMILTONIAN_APPLY, OP_CHEBYSHEV_FILTER, OP_PROJECT, OP_ROTATE = 0, 1, 2, 3
+OP_GRADIENT_PROJECT, OP_NONLOCAL_FORCE, OP_EIGENSOLVE = 4, 5, 6
 
 EXPORTS = ["sparc_gpu_create", "sparc_gpu_destroy", "sparc_gpu_set_veff", "sparc_gpu_workspace_bytes",
            "sparc_gpu_set_workspace_size",
            "sparc_gpu_hamiltonian_apply", "sparc_gpu_chebyshev_filter", "sparc_gpu_project",
-           "sparc_gpu_rotate", "sparc_gpu_fill_uniform", "sparc_gpu_set_option", "sparc_gpu_get_info", "sparc_gpu_probe_peak",
+           "sparc_gpu_rotate", "sparc_gpu_chefsi_step_host", "sparc_gpu_gradient",
+           "sparc_gpu_nl_project", "sparc_gpu_gradient_project", "sparc_gpu_nonlocal_force", "sparc_gpu_eigensolve", "sparc_gpu_fill_uniform", "sparc_gpu_set_option", "sparc_gpu_get_info", "sparc_gpu_probe_peak",
            "sparc_gpu_error_string", "sparc_gpu_version"]
 
 
@@ -65,6 +67,12 @@ def load_library(build_if_missing: bool = True):
     lib.sparc_gpu_chebyshev_filter.argtypes = [P, P, I64, I64, I, D, D, D, I64, P, P]
     lib.sparc_gpu_project.argtypes = [P, P, I64, I64, P, P, I64, P, P]
     lib.sparc_gpu_rotate.argtypes = [P, P, I64, I64, P, I64, P, P]
+    lib.sparc_gpu_chefsi_step_host.argtypes = [P, P, P, I64, I64, I, D, D, D, P, P, P, P, I64, P, I64, I64, P, P]
+    lib.sparc_gpu_gradient.argtypes = [P, I, P, I64, P, I64, I64, P]
+    lib.sparc_gpu_nl_project.argtypes = [P, P, I64, I64, P, P]
+    lib.sparc_gpu_gradient_project.argtypes = [P, I, P, I64, I64, P, I64, P, P]
+    lib.sparc_gpu_nonlocal_force.argtypes = [P, P, I64, I64, P, P, I64, P, P]
+    lib.sparc_gpu_eigensolve.argtypes = [P, I64, P, P, P, P, P, P, P]
     lib.sparc_gpu_fill_uniform.argtypes = [P, I64, C.c_uint64, C.c_uint64, C.c_uint64, D, D, I, P]
     lib.sparc_gpu_probe_peak.argtypes = [I, I, C.POINTER(D), P, I64, P]
     lib.sparc_gpu_set_option.argtypes = [P, C.c_char_p, I64]
@@ -153,6 +161,7 @@ class SparcGpu:
             d.n[k], d.h[k], d.bc[k] = int(wl.n[k]), float(wl.h[k]), int(wl.bc[k])
         d.fd_order = int(wl.fd_order)
         d.n_atoms = int(keep["n_proj"].shape[0])
+        self.n_atoms = d.n_atoms
         for name, arr in keep.items():
             setattr(d, name, arr.ctypes.data if arr.size else None)
         veff = None
@@ -291,6 +300,90 @@ class SparcGpu:
         for st in (s_in, s_run, s_out):
             st.synchronize()
         return host_out
+
+    def chefsi_step_host(self, host_psi, Q_host, Hs_host, Ms_host, degree: int, a: float, b: float, a0: float,
+                         psi_dev=None, mats_dev=None, col_block: int = 0, row_panel: int = 0, host_out=None):
+        """sparc_gpu_chefsi_step_host: filter -> project -> rotate on a block in (pinned) HOST memory.  host_psi:
+        (ns, ld) CPU tensor, overwritten with the rotated block unless host_out is given; Q_host, Hs_host, Ms_host: (ns, ns)
+        CPU tensors.  psi_dev / mats_dev: optional device scratch to reuse.  Synchronises."""
+        torch = _torch()
+        ns, ld = int(host_psi.shape[0]), int(host_psi.shape[1])
+        host_out = host_psi if host_out is None else host_out
+        for t in (host_psi, host_out, Q_host, Hs_host, Ms_host):
+            assert (not t.is_cuda) and t.dtype == torch.float64 and t.is_contiguous()
+        assert ld >= self.nd and host_out.shape == host_psi.shape and Q_host.shape == (ns, ns)
+        dev = torch.device("cuda", self.device)
+        if psi_dev is None:
+            psi_dev = torch.empty((ns, self.nd), dtype=torch.float64, device=dev)
+        if mats_dev is None:
+            mats_dev = torch.empty(3 * ns * ns, dtype=torch.float64, device=dev)
+        pp, ldd, _ = self._mat(psi_dev, "psi_dev")
+        need = max(self.workspace_bytes(OP_CHEBYSHEV_FILTER, ns, col_block), self.workspace_bytes(OP_PROJECT, ns, col_block),
+                   self.workspace_bytes(OP_ROTATE, ns, row_panel))
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = None
+            self._ws = torch.empty(need, dtype=torch.uint8, device=dev)
+            _check(self.lib.sparc_gpu_set_workspace_size(self._ctx, self._ws.numel()), "set_workspace_size")
+        _check(self.lib.sparc_gpu_chefsi_step_host(
+            self._ctx, C.c_void_p(host_psi.data_ptr()), C.c_void_p(host_out.data_ptr()), ld, ns, int(degree), float(a),
+            float(b), float(a0), C.c_void_p(Q_host.data_ptr()), C.c_void_p(Hs_host.data_ptr()),
+            C.c_void_p(Ms_host.data_ptr()), pp, ldd, C.c_void_p(mats_dev.data_ptr()), int(col_block), int(row_panel),
+            C.c_void_p(self._ws.data_ptr()), self._stream()), "chefsi_step_host")
+        return host_out
+
+    # ---- NEXT-3: gradient stencil, projector contraction, nonlocal force --------------------------
+    def gradient(self, X, axis: int, Y=None):
+        torch = _torch()
+        xp, ldx, ncols = self._mat(X, "X")
+        if Y is None:
+            Y = torch.empty_like(X)
+        yp, ldy, _ = self._mat(Y, "Y")
+        _check(self.lib.sparc_gpu_gradient(self._ctx, int(axis), xp, ldx, yp, ldy, ncols, self._stream()), "gradient")
+        return Y
+
+    def nl_project(self, X):
+        """W = chi^T X as an (ncols, n_proj_total) tensor holding the column-major n_proj_total x ncols matrix."""
+        torch = _torch()
+        xp, ldx, ncols = self._mat(X, "X")
+        W = torch.zeros((ncols, self.get_info("n_proj_total")), dtype=torch.float64, device=X.device)
+        _check(self.lib.sparc_gpu_nl_project(self._ctx, xp, ldx, ncols, C.c_void_p(W.data_ptr()), self._stream()), "nl_project")
+        return W
+
+    def gradient_project(self, X, axis: int, col_block: int = 0):
+        torch = _torch()
+        xp, ldx, ncols = self._mat(X, "X")
+        W = torch.zeros((ncols, self.get_info("n_proj_total")), dtype=torch.float64, device=X.device)
+        ws = self._workspace(OP_GRADIENT_PROJECT, ncols, col_block)
+        _check(self.lib.sparc_gpu_gradient_project(self._ctx, int(axis), xp, ldx, ncols, C.c_void_p(W.data_ptr()),
+                                                   int(col_block), ws, self._stream()), "gradient_project")
+        return W
+
+    def nonlocal_force(self, Psi, occ, col_block: int = 0):
+        """F (n_atoms, 3) = nonlocal Hellmann-Feynman force; occ: (ns,) float64 CUDA tensor."""
+        torch = _torch()
+        pp, ld, ns = self._mat(Psi, "Psi")
+        assert occ.is_cuda and occ.dtype == torch.float64 and occ.numel() == ns and occ.is_contiguous()
+        F = torch.empty((max(self.n_atoms, 1), 3), dtype=torch.float64, device=Psi.device)
+        ws = self._workspace(OP_NONLOCAL_FORCE, ns, col_block)
+        _check(self.lib.sparc_gpu_nonlocal_force(self._ctx, pp, ld, ns, C.c_void_p(occ.data_ptr()),
+                                                 C.c_void_p(F.data_ptr()), int(col_block), ws, self._stream()), "nonlocal_force")
+        return F[:self.n_atoms]
+
+    # ---- NEXT-1: subspace eigenproblem on the device ---------------------------------------------------
+    def eigensolve(self, Hs, Ms):
+        """Hs Z = Ms Z D on the device: returns (D (n,), Z (n, n) tensor holding the column-major matrix, info (2,) int32:
+        status, sweeps).  Nothing is synchronised; read `info` after a stream sync."""
+        torch = _torch()
+        n = int(Hs.shape[0])
+        assert Hs.is_cuda and Ms.is_cuda and Hs.shape == (n, n) and Ms.shape == (n, n) and Hs.is_contiguous() and Ms.is_contiguous()
+        Z = torch.empty((n, n), dtype=torch.float64, device=Hs.device)
+        D = torch.empty(n, dtype=torch.float64, device=Hs.device)
+        info = torch.zeros(2, dtype=torch.int32, device=Hs.device)
+        ws = self._workspace(OP_EIGENSOLVE, n, 0)
+        _check(self.lib.sparc_gpu_eigensolve(self._ctx, n, C.c_void_p(Hs.data_ptr()), C.c_void_p(Ms.data_ptr()),
+                                             C.c_void_p(Z.data_ptr()), C.c_void_p(D.data_ptr()), C.c_void_p(info.data_ptr()), ws,
+                                             self._stream()), "eigensolve")
+        return D, Z, info
 
     def project(self, Psi, col_block: int = 0, Hs=None, Ms=None):
         torch = _torch()

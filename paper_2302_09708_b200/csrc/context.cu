@@ -79,6 +79,17 @@ void fd_weights_host(int r, double *w)
     w[0] = (double)w0;
 }
 
+// central FD weights of the first derivative, radius r (reading R21): w_p = (-1)^{p+1} (r!)^2 / (p (r-p)! (r+p)!)
+void fd1_weights_host(int r, double *w)
+{
+    w[0] = 0.0;
+    for (int p = 1; p <= r; ++p) {
+        long double ratio = 1.0L;
+        for (int j = 1; j <= p; ++j) ratio *= (long double)(r - p + j) / (long double)(r + j);
+        w[p] = (double)(((p & 1) ? ratio : -ratio) / (long double)p);
+    }
+}
+
 template <typename T>
 int upload(T **dst, const T *src, size_t count)
 {
@@ -94,6 +105,7 @@ void free_tables(sparc_gpu_ctx *c)
     cudaFree(c->d_supp_ptr); cudaFree(c->d_supp_idx); cudaFree(c->d_n_proj); cudaFree(c->d_proj_ofs);
     cudaFree(c->d_chi_ptr); cudaFree(c->d_chi); cudaFree(c->d_gamma); cudaFree(c->d_cov_idx);
     cudaFree(c->d_cov_ptr); cudaFree(c->d_cov_ent); cudaFree(c->d_veff);
+    for (int k = 0; k < 2; ++k) if (c->copy_stream[k]) { cudaStreamDestroy(c->copy_stream[k]); c->copy_stream[k] = nullptr; }
     nlb_free(c);
 }
 
@@ -126,68 +138,6 @@ int validate_desc(const sparc_gpu_desc *d)
         }
     }
     return SPARC_GPU_SUCCESS;
-}
-
-struct WsLayout {
-    int64_t block;       // column block / row panel actually used
-    int64_t ldw;         // leading dimension of the work block
-    int64_t off_w, off_d, off_g;
-    int64_t total;
-};
-
-int64_t default_col_block(const sparc_gpu_ctx *c, int64_t ns) { (void)c; return std::min<int64_t>(ns, 1024); }
-
-int64_t default_row_panel(const sparc_gpu_ctx *c, int64_t ns)
-{
-    // stage of at most ~2 GiB, at least 128 rows, multiple of 128
-    int64_t r = (int64_t)(2048LL << 20) / (8 * std::max<int64_t>(ns, 1));
-    r = std::max<int64_t>(128, r / 128 * 128);
-    return std::min<int64_t>(r, round_up_i64(c->nd, 128));
-}
-
-int ws_layout(const sparc_gpu_ctx *c, int op, int64_t ns, int64_t block, WsLayout *L)
-{
-    if (ns < 0) return SPARC_GPU_INVALID_ARG;
-    memset(L, 0, sizeof(*L));
-    const int64_t A = 256;
-    int64_t off = 0;
-    switch (op) {
-    case SPARC_GPU_OP_HAMILTONIAN_APPLY:
-    case SPARC_GPU_OP_CHEBYSHEV_FILTER:
-    case SPARC_GPU_OP_PROJECT: {
-        int64_t cb = block > 0 ? std::min(block, std::max<int64_t>(ns, 1)) : default_col_block(c, std::max<int64_t>(ns, 1));
-        L->block = cb;
-        L->ldw = round_up_i64(c->nd, 16);
-        L->off_w = off;
-        if (op != SPARC_GPU_OP_HAMILTONIAN_APPLY) off += round_up_i64(L->ldw * cb * 8, A);
-        L->off_d = off;
-        off += round_up_i64(2 * (int64_t)std::max(c->n_proj_total, 1) * nlb_c_cols(cb) * 8, A);
-        L->off_g = off;
-        if (op == SPARC_GPU_OP_PROJECT) {
-            off += round_up_i64(std::max(gemm_tn_ws_bytes(c, ns, cb, c->nd), gemm_tn_ws_bytes(c, ns, ns, c->nd)), A);
-        }
-        break;
-    }
-    case SPARC_GPU_OP_ROTATE: {
-        int64_t rp = block > 0 ? block : default_row_panel(c, ns);
-        rp = std::min<int64_t>(rp, c->nd);
-        L->block = rp;
-        L->ldw = round_up_i64(rp, 16);
-        L->off_w = off;
-        off += round_up_i64(L->ldw * std::max<int64_t>(ns, 1) * 8, A);
-        break;
-    }
-    default:
-        return SPARC_GPU_INVALID_ARG;
-    }
-    L->total = std::max<int64_t>(off, A);
-    return SPARC_GPU_SUCCESS;
-}
-
-// the caller declared the size of its workspace (sparc_gpu_set_workspace_size): refuse a call that would overrun it
-int ws_check(const sparc_gpu_ctx *c, const WsLayout &L)
-{
-    return (c->ws_bytes > 0 && L.total > c->ws_bytes) ? SPARC_GPU_WORKSPACE_TOO_SMALL : SPARC_GPU_SUCCESS;
 }
 
 // Out = alpha (H_loc X + shift X) + beta Prev on one column block: the fused local pass (stencil + Veff + axpy).
@@ -249,6 +199,103 @@ int h_apply_block(sparc_gpu_ctx *c, const double *X, int64_t ldx, double *Y, int
 
 }  // namespace
 
+
+static int64_t default_col_block(const sparc_gpu_ctx *c, int64_t ns) { (void)c; return std::min<int64_t>(ns, 1024); }
+
+static int64_t default_row_panel(const sparc_gpu_ctx *c, int64_t ns)
+{
+    // stage of at most ~2 GiB, at least 128 rows, multiple of 128
+    int64_t r = (int64_t)(2048LL << 20) / (8 * std::max<int64_t>(ns, 1));
+    r = std::max<int64_t>(128, r / 128 * 128);
+    return std::min<int64_t>(r, round_up_i64(c->nd, 128));
+}
+
+int ws_layout(const sparc_gpu_ctx *c, int op, int64_t ns, int64_t block, WsLayout *L)
+{
+    if (ns < 0) return SPARC_GPU_INVALID_ARG;
+    memset(L, 0, sizeof(*L));
+    const int64_t A = 256;
+    int64_t off = 0;
+    switch (op) {
+    case SPARC_GPU_OP_HAMILTONIAN_APPLY:
+    case SPARC_GPU_OP_CHEBYSHEV_FILTER:
+    case SPARC_GPU_OP_PROJECT: {
+        int64_t cb = block > 0 ? std::min(block, std::max<int64_t>(ns, 1)) : default_col_block(c, std::max<int64_t>(ns, 1));
+        L->block = cb;
+        L->ldw = round_up_i64(c->nd, 16);
+        L->off_w = off;
+        if (op != SPARC_GPU_OP_HAMILTONIAN_APPLY) off += round_up_i64(L->ldw * cb * 8, A);
+        L->off_d = off;
+        off += round_up_i64(2 * (int64_t)std::max(c->n_proj_total, 1) * nlb_c_cols(cb) * 8, A);
+        L->off_g = off;
+        if (op == SPARC_GPU_OP_PROJECT) {
+            off += round_up_i64(std::max(gemm_tn_ws_bytes(c, ns, cb, c->nd), gemm_tn_ws_bytes(c, ns, ns, c->nd)), A);
+        }
+        break;
+    }
+    case SPARC_GPU_OP_GRADIENT_PROJECT:
+    case SPARC_GPU_OP_NONLOCAL_FORCE: {
+        // one gradient block Y = D_a X, and (force) the two projection blocks W = chi^T X, G = chi^T Y
+        int64_t cb = block > 0 ? std::min(block, std::max<int64_t>(ns, 1)) : default_col_block(c, std::max<int64_t>(ns, 1));
+        L->block = cb;
+        L->ldw = round_up_i64(c->nd, 16);
+        L->off_w = off;
+        off += round_up_i64(L->ldw * cb * 8, A);
+        L->off_d = off;
+        if (op == SPARC_GPU_OP_NONLOCAL_FORCE) off += round_up_i64(2 * (int64_t)std::max(c->n_proj_total, 1) * cb * 8, A);
+        break;
+    }
+    case SPARC_GPU_OP_EIGENSOLVE: {
+        // A, V (n x n each, the Jacobi iterate and the accumulated rotations), L (Cholesky factor), 2 n scalars
+        const int64_t n = std::max<int64_t>(ns, 1), np = round_up_i64(n, 32);
+        L->block = np;
+        L->ldw = np;
+        L->off_w = off;
+        off += round_up_i64(4 * np * np * 8 + 8 * np * 8 + 4096, A);
+        break;
+    }
+    case SPARC_GPU_OP_ROTATE: {
+        int64_t rp = block > 0 ? block : default_row_panel(c, ns);
+        rp = std::min<int64_t>(rp, c->nd);
+        L->block = rp;
+        L->ldw = round_up_i64(rp, 16);
+        L->off_w = off;
+        off += round_up_i64(L->ldw * std::max<int64_t>(ns, 1) * 8, A);
+        break;
+    }
+    default:
+        return SPARC_GPU_INVALID_ARG;
+    }
+    L->total = std::max<int64_t>(off, A);
+    return SPARC_GPU_SUCCESS;
+}
+
+// the caller declared the size of its workspace (sparc_gpu_set_workspace_size): refuse a call that would overrun it
+int ws_check(const sparc_gpu_ctx *c, const WsLayout &L)
+{
+    return (c->ws_bytes > 0 && L.total > c->ws_bytes) ? SPARC_GPU_WORKSPACE_TOO_SMALL : SPARC_GPU_SUCCESS;
+}
+
+
+// row panel and stage pitch a rotation of ns columns uses (and the workspace check that goes with them)
+int rotate_layout(const sparc_gpu_ctx *c, int64_t ns, int64_t row_panel, int64_t *rp, int64_t *ldw)
+{
+    WsLayout L;
+    SPARC_TRY(ws_layout(c, SPARC_GPU_OP_ROTATE, ns, row_panel, &L));
+    SPARC_TRY(ws_check(c, L));
+    *rp = L.block; *ldw = L.ldw;
+    return SPARC_GPU_SUCCESS;
+}
+
+// rows [0, nr) of Psi_rows <- the same rows times Q, staged through T (the product must not overwrite rows it still reads)
+int rotate_panel(sparc_gpu_ctx *c, double *Psi_rows, int64_t ld, int64_t nr, int64_t ns, const double *Q, double *T,
+                 int64_t ldw, cudaStream_t st)
+{
+    SPARC_TRY(launch_gemm_nn(c, Psi_rows, ld, Q, ns, T, ldw, nr, ns, ns, st));
+    SPARC_TRY(launch_copy_2d(c, Psi_rows, ld, T, ldw, nr, ns, st));
+    return SPARC_GPU_SUCCESS;
+}
+
 extern "C" {
 
 const char *sparc_gpu_version(void) { return "sparc_gpu 0.1.0 (sm_100a)"; }
@@ -291,6 +338,7 @@ int sparc_gpu_create(const sparc_gpu_desc *desc, sparc_gpu_ctx **out)
     c->nd = (int64_t)desc->n[0] * desc->n[1] * desc->n[2];
     c->prof = new (std::nothrow) ProfState();
     fd_weights_host(c->radius, c->w);
+    fd1_weights_host(c->radius, c->w1);
     double isum = 0.0;
     for (int p = 0; p <= SPARC_MAX_RADIUS; ++p) { c->coef.cx[p] = c->coef.cy[p] = c->coef.cz[p] = 0.0; }
     for (int p = 1; p <= c->radius; ++p) {
@@ -585,8 +633,7 @@ int sparc_gpu_rotate(sparc_gpu_ctx *ctx, double *Psi, int64_t ld, int64_t ns, co
     double *T = (double *)((char *)ws + L.off_w);
     for (int64_t r0 = 0; r0 < ctx->nd; r0 += L.block) {
         const int64_t nr = std::min(L.block, ctx->nd - r0);
-        SPARC_TRY(launch_gemm_nn(ctx, Psi + r0, ld, Q, ns, T, L.ldw, nr, ns, ns, st));
-        SPARC_TRY(launch_copy_2d(ctx, Psi + r0, ld, T, L.ldw, nr, ns, st));
+        SPARC_TRY(rotate_panel(ctx, Psi + r0, ld, nr, ns, Q, T, L.ldw, st));
     }
     return SPARC_GPU_SUCCESS;
 }

@@ -104,6 +104,8 @@ struct sparc_gpu_ctx {
     uint64_t func_attr_done = 0;   // kernel variants whose dynamic shared-memory attribute is set (nonlocal_brick.cu)
     // driver entry point for tensor-map encoding (resolved at create; NULL if unavailable)
     void *fn_encode_tiled = nullptr;
+    // copy streams of the host-buffer entry point (step_host.cu), created on first use
+    cudaStream_t copy_stream[2] = {nullptr, nullptr};
     // optional per-kernel CUDA-event timing (option "profile"); NULL when off
     struct ProfState *prof = nullptr;
 };
@@ -146,6 +148,16 @@ void prof_end(sparc_gpu_ctx *ctx, int kind, cudaStream_t st);
 
 static inline int64_t round_up_i64(int64_t v, int64_t m) { return (v + m - 1) / m * m; }
 
+// Carving of the caller's workspace for one operator call (context.cu).
+struct WsLayout {
+    int64_t block;       // column block / row panel actually used
+    int64_t ldw;         // leading dimension of the work block
+    int64_t off_w, off_d, off_g;
+    int64_t total;
+};
+int ws_layout(const sparc_gpu_ctx *c, int op, int64_t ns, int64_t block, WsLayout *L);
+int ws_check(const sparc_gpu_ctx *c, const WsLayout &L);
+
 // ---- kernel launchers (each returns a sparc_gpu_status and bumps ctx->kernel_launches) ----------
 
 // Out = alpha * (H_loc X + shift X) + beta * Prev   (Prev may be NULL when beta == 0; Prev may alias Out)
@@ -168,6 +180,8 @@ bool stencil_tma_supported(const sparc_gpu_ctx *ctx, const double *X, int64_t ld
 // D[q, col] = scale * gamma[q] * sum_t chi[t, q] X[idx[t], col]     (D: n_proj_total x ncols, ld = n_proj_total)
 int launch_nl_project(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, int64_t ncols, double scale,
                       double *D, cudaStream_t st);
+// W[q, col] = sum_t chi[t, q] X[idx[t], col]   (no Gamma; W: n_proj_total x ncols, ld = n_proj_total)
+int launch_nl_project_raw(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, int64_t ncols, double *W, cudaStream_t st);
 // Out[i, col] += sum_{(J,t) covering i} sum_q chi_J[t, q] D[ofs_J + q, col]
 int launch_nl_pull(sparc_gpu_ctx *ctx, const double *D, double *Out, int64_t ldo, int64_t ncols,
                    cudaStream_t st);
@@ -200,6 +214,10 @@ int launch_mirror_upper(sparc_gpu_ctx *ctx, double *C, int64_t ldc, int64_t n, c
 // C (M x N, ldc) = A B, A: M x K col-major (lda), B: K x N col-major (ldb)
 int launch_gemm_nn(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const double *B, int64_t ldb,
                    double *C, int64_t ldc, int64_t M, int64_t N, int64_t K, cudaStream_t st);
+// rotation by row panels (context.cu): panel size / stage pitch for ns columns, and one panel Psi_rows <- Psi_rows Q
+int rotate_layout(const sparc_gpu_ctx *ctx, int64_t ns, int64_t row_panel, int64_t *rp, int64_t *ldw);
+int rotate_panel(sparc_gpu_ctx *ctx, double *Psi_rows, int64_t ld, int64_t nr, int64_t ns, const double *Q, double *T,
+                 int64_t ldw, cudaStream_t st);
 // dst (rows x cols, ldd) = src (rows x cols, lds)
 int launch_copy_2d(sparc_gpu_ctx *ctx, double *dst, int64_t ldd, const double *src, int64_t lds,
                    int64_t rows, int64_t cols, cudaStream_t st);

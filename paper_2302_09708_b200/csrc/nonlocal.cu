@@ -67,7 +67,7 @@ nl_project_kernel(const int64_t *__restrict__ supp_ptr, const int32_t *__restric
                 double v = acc[q][c];
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-                if (lane == 0 && col0 + c < ncols) D[(int64_t)(po + q) + (col0 + c) * (int64_t)ldD] = scale * gamma[po + q] * v;
+                if (lane == 0 && col0 + c < ncols) D[(int64_t)(po + q) + (col0 + c) * (int64_t)ldD] = gamma ? scale * gamma[po + q] * v : v;
             }
         }
     }
@@ -251,8 +251,8 @@ nl_fused_kernel(const int64_t *__restrict__ supp_ptr, const int32_t *__restrict_
 
 }  // namespace
 
-int launch_nl_project(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, int64_t ncols, double scale, double *D,
-                      cudaStream_t st)
+static int nl_project_impl(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, int64_t ncols, double scale, const double *gamma,
+                           double *D, cudaStream_t st)
 {
     const int cols_per_cta = NLP_WARPS * NLP_COLS;
     const int64_t max_y = 65535;
@@ -263,7 +263,7 @@ int launch_nl_project(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, int64_t 
         double *Db = D + j0 * (int64_t)ctx->n_proj_total;
 #define NLP_LAUNCH(PM)                                                                                         \
         nl_project_kernel<PM><<<grid, NLP_WARPS * 32, 0, st>>>(ctx->d_supp_ptr, ctx->d_supp_idx, ctx->d_n_proj, \
-            ctx->d_proj_ofs, ctx->d_chi_ptr, ctx->d_chi, ctx->d_gamma, Xb, ldx, nb, scale, Db, ctx->n_proj_total)
+            ctx->d_proj_ofs, ctx->d_chi_ptr, ctx->d_chi, gamma, Xb, ldx, nb, scale, Db, ctx->n_proj_total)
         prof_begin(ctx, KK_NL_PROJECT, st);
         if (ctx->max_proj <= 4) NLP_LAUNCH(4);
         else if (ctx->max_proj <= 9) NLP_LAUNCH(9);
@@ -273,6 +273,18 @@ int launch_nl_project(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, int64_t 
     }
     SPARC_CUDA_TRY(cudaGetLastError());
     return SPARC_GPU_SUCCESS;
+}
+
+int launch_nl_project(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, int64_t ncols, double scale, double *D,
+                      cudaStream_t st)
+{
+    return nl_project_impl(ctx, X, ldx, ncols, scale, ctx->d_gamma, D, st);
+}
+
+// W = chi^T X (no Gamma): the projector contraction of the force (gradient.cu)
+int launch_nl_project_raw(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, int64_t ncols, double *W, cudaStream_t st)
+{
+    return nl_project_impl(ctx, X, ldx, ncols, 1.0, nullptr, W, st);
 }
 
 int launch_nl_pull(sparc_gpu_ctx *ctx, const double *D, double *Out, int64_t ldo, int64_t ncols, cudaStream_t st)
