@@ -303,6 +303,8 @@ def bench_config(env, config, steps, warmup, *, col_block=0, stencil_path=0, ste
                        "divides by the filter time alone; compare step_s with ms_per_step"
                        + ("" if ns_e == ns else f"; host memory bounds the sample to the first {ns_e} of {ns} columns")}
         del host_psi, Q_host, Hs_host, Ms_host, mats
+        if hasattr(torch._C, "_host_emptyCache"):
+            torch._C._host_emptyCache()           # hand the pinned block back to the OS (the next workload sizes its own)
 
     # ---- rooflines: per-launch CUDA events inside the library (option "profile"), same launch configuration ----
     roofline = None

@@ -30,7 +30,7 @@ def api():
 
 @pytest.fixture(scope="module")
 def g(api):
-    wl = wlmod.make_custom("eig_ctx", (12, 12, 12), (0.5,) * 3, (0, 0, 0), 2, 2, np.zeros((0, 3)), [], 2.0, seed=3)
+    wl = wlmod.make_custom("eig_ctx", (14, 14, 14), (0.5,) * 3, (0, 0, 0), 2, 2, np.zeros((0, 3)), [], 2.0, seed=3)
     ctx = api.SparcGpu(wl)
     yield ctx
     ctx.close()

@@ -73,7 +73,7 @@ def test_gradient_project_force_small(torch, api, wl):
 def test_lower_orders_and_degenerate(torch, api):
     pos = np.array([[1.0, 2.0, 3.0]])
     for fd_order in (2, 6):
-        wl = wlmod.make_custom(f"g_fd{fd_order}", (9, 8, 7), (0.5, 0.5, 0.5), (0, 1, 0), 3, 2, pos, [4], 2.0, seed=33,
+        wl = wlmod.make_custom(f"g_fd{fd_order}", (9, 8, 7), (0.5, 0.5, 0.5), (0, 1, 0), 3, 2, pos, [4], 1.5, seed=33,
                                fd_order=fd_order)
         g = api.SparcGpu(wl)
         F = orc.Forces(wl)
@@ -82,7 +82,7 @@ def test_lower_orders_and_degenerate(torch, api):
         for axis in range(3):
             assert col_err(api.colmajor_to_numpy(g.gradient(Xg, axis), wl.nd), F.gradient(X, axis)) <= 1e-13
         g.close()
-    wl = wlmod.make_custom("g_noatoms", (12, 12, 12), (0.5,) * 3, (0, 0, 0), 2, 2, np.zeros((0, 3)), [], 2.0, seed=34)
+    wl = wlmod.make_custom("g_noatoms", (14, 14, 14), (0.5,) * 3, (0, 0, 0), 2, 2, np.zeros((0, 3)), [], 2.0, seed=34)
     g = api.SparcGpu(wl)
     Xg = api.colmajor_from_numpy(wl.psi_columns(range(2)))
     assert g.nonlocal_force(Xg, torch.ones(2, dtype=torch.float64, device="cuda")).shape[0] == 0
