@@ -67,7 +67,11 @@ typedef enum {
     SPARC_GPU_OP_ROTATE = 3,
     SPARC_GPU_OP_GRADIENT_PROJECT = 4,
     SPARC_GPU_OP_NONLOCAL_FORCE = 5,
-    SPARC_GPU_OP_EIGENSOLVE = 6
+    SPARC_GPU_OP_EIGENSOLVE = 6,
+    SPARC_GPU_OP_HAMILTONIAN_APPLY_K = 7,
+    SPARC_GPU_OP_CHEBYSHEV_FILTER_K = 8,
+    SPARC_GPU_OP_PROJECT_K = 9,
+    SPARC_GPU_OP_ROTATE_K = 10
 } sparc_gpu_op;
 
 /* Problem description (all pointers HOST, copied at create).  PAPER.md:118 "The matrix X, effective
@@ -169,6 +173,32 @@ int sparc_gpu_nonlocal_force(sparc_gpu_ctx *ctx, const double *Psi_dev, int64_t 
  * Workspace op EIGENSOLVE with ns = n.  n <= 12800 (a column pair must fit shared memory), else UNSUPPORTED. */
 int sparc_gpu_eigensolve(sparc_gpu_ctx *ctx, int64_t n, const double *Hs_dev, const double *Ms_dev, double *Z_dev,
                          double *D_dev, int32_t *info_dev, void *ws_dev, void *stream);
+
+/* ---- complex (k-point) variant ------------------------------------------------------------
+ * PAPER.md:35 ("complex-valued ... Bloch wavevectors"), 126 / 146 / 166 (the Zgemm forms), 176 (Monkhorst-Pack grids).
+ * Complex arrays are interleaved (re, im) doubles; leading dimensions and ns x ns sizes count COMPLEX elements.
+ * Readings R24-R27: psi(r + L_a e_a) = exp(i theta_a) psi(r) on a periodic axis (theta_a = k_a L_a; ignored on Dirichlet axes):
+ * a stencil tap wrapping through the upper (lower) face of axis a carries exp(+i theta_a) (exp(-i theta_a)); a support row
+ * folded into the cell by the image shift w_a in {-1, 0, +1} per axis acts as chi~[t, q] = chi[t, q] exp(-i sum_a w_a theta_a),
+ * V_nl = sum_J chi~_J Gamma_J chi~_J^H (chi real). */
+
+/* Select the k-point of the following *_k calls.  theta: 3 doubles (HOST); supp_shift: int8 [supp_total][3] image shifts of the
+ * support rows in the order of desc->supp_idx (HOST), or NULL (all zero).  Blocking (synchronises the device, uploads tables). */
+int sparc_gpu_set_kpoint(sparc_gpu_ctx *ctx, const double *theta, const int8_t *supp_shift);
+
+/* Y = H(k) X on complex columns (workspace op HAMILTONIAN_APPLY_K). */
+int sparc_gpu_hamiltonian_apply_k(sparc_gpu_ctx *ctx, const double *X_dev, int64_t ldx, double *Y_dev, int64_t ldy,
+                                  int64_t ncols, void *ws_dev, void *stream);
+/* In-place scaled Chebyshev filter with H(k): the recurrence of sparc_gpu_chebyshev_filter on complex columns. */
+int sparc_gpu_chebyshev_filter_k(sparc_gpu_ctx *ctx, double *Psi_dev, int64_t ld, int64_t ns, int degree, double a,
+                                 double b, double a0, int64_t col_block, void *ws_dev, void *stream);
+/* Hs = Psi^H (H(k) Psi), Ms = Psi^H Psi: complex ns x ns column-major, Hermitian up to rounding, both triangles filled
+ * (PAPER.md:146 cublasZgemm with the conjugate transpose). */
+int sparc_gpu_project_k(sparc_gpu_ctx *ctx, const double *Psi_dev, int64_t ld, int64_t ns, double *Hs_dev, double *Ms_dev,
+                        int64_t col_block, void *ws_dev, void *stream);
+/* Psi <- Psi Q in place by row panels, Q complex ns x ns (PAPER.md:166 cublasZgemm). */
+int sparc_gpu_rotate_k(sparc_gpu_ctx *ctx, double *Psi_dev, int64_t ld, int64_t ns, const double *Q_dev, int64_t row_panel,
+                       void *ws_dev, void *stream);
 
 /* One whole CheFSI step -- filter, project, rotate -- for a block that lives in HOST memory (what the paper's code does
  * around every step with cublasSet/GetVector: PAPER.md:118, 128, 138, 146, 158, 166), with the PCIe copies overlapped with

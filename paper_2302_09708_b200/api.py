@@ -22,12 +22,15 @@ _lib = None
 
 OP_HAMILTONIAN_APPLY, OP_CHEBYSHEV_FILTER, OP_PROJECT, OP_ROTATE = 0, 1, 2, 3
 OP_GRADIENT_PROJECT, OP_NONLOCAL_FORCE, OP_EIGENSOLVE = 4, 5, 6
+OP_HAMILTONIAN_APPLY_K, OP_CHEBYSHEV_FILTER_K, OP_PROJECT_K, OP_ROTATE_K = 7, 8, 9, 10
 
 EXPORTS = ["sparc_gpu_create", "sparc_gpu_destroy", "sparc_gpu_set_veff", "sparc_gpu_workspace_bytes",
            "sparc_gpu_set_workspace_size",
            "sparc_gpu_hamiltonian_apply", "sparc_gpu_chebyshev_filter", "sparc_gpu_project",
            "sparc_gpu_rotate", "sparc_gpu_chefsi_step_host", "sparc_gpu_gradient",
-           "sparc_gpu_nl_project", "sparc_gpu_gradient_project", "sparc_gpu_nonlocal_force", "sparc_gpu_eigensolve", "sparc_gpu_fill_uniform", "sparc_gpu_set_option", "sparc_gpu_get_info", "sparc_gpu_probe_peak",
+           "sparc_gpu_nl_project", "sparc_gpu_gradient_project", "sparc_gpu_nonlocal_force", "sparc_gpu_eigensolve", "sparc_gpu_set_kpoint",
+           "sparc_gpu_hamiltonian_apply_k", "sparc_gpu_chebyshev_filter_k", "sparc_gpu_project_k", "sparc_gpu_rotate_k",
+           "sparc_gpu_fill_uniform", "sparc_gpu_set_option", "sparc_gpu_get_info", "sparc_gpu_probe_peak",
            "sparc_gpu_error_string", "sparc_gpu_version"]
 
 
@@ -73,6 +76,11 @@ def load_library(build_if_missing: bool = True):
     lib.sparc_gpu_gradient_project.argtypes = [P, I, P, I64, I64, P, I64, P, P]
     lib.sparc_gpu_nonlocal_force.argtypes = [P, P, I64, I64, P, P, I64, P, P]
     lib.sparc_gpu_eigensolve.argtypes = [P, I64, P, P, P, P, P, P, P]
+    lib.sparc_gpu_set_kpoint.argtypes = [P, P, P]
+    lib.sparc_gpu_hamiltonian_apply_k.argtypes = [P, P, I64, P, I64, I64, P, P]
+    lib.sparc_gpu_chebyshev_filter_k.argtypes = [P, P, I64, I64, I, D, D, D, I64, P, P]
+    lib.sparc_gpu_project_k.argtypes = [P, P, I64, I64, P, P, I64, P, P]
+    lib.sparc_gpu_rotate_k.argtypes = [P, P, I64, I64, P, I64, P, P]
     lib.sparc_gpu_fill_uniform.argtypes = [P, I64, C.c_uint64, C.c_uint64, C.c_uint64, D, D, I, P]
     lib.sparc_gpu_probe_peak.argtypes = [I, I, C.POINTER(D), P, I64, P]
     lib.sparc_gpu_set_option.argtypes = [P, C.c_char_p, I64]
@@ -384,6 +392,59 @@ class SparcGpu:
                                              C.c_void_p(Z.data_ptr()), C.c_void_p(D.data_ptr()), C.c_void_p(info.data_ptr()), ws,
                                              self._stream()), "eigensolve")
         return D, Z, info
+
+    # ---- NEXT-4: complex (k-point) variant; complex matrices are torch.complex128 tensors (ncols, ld) ----------
+    def set_kpoint(self, theta, supp_shift=None):
+        th = (C.c_double * 3)(*[float(t) for t in theta])
+        sh = None
+        if supp_shift is not None:
+            self._shift = np.ascontiguousarray(supp_shift, dtype=np.int8)
+            sh = self._shift.ctypes.data
+        _check(self.lib.sparc_gpu_set_kpoint(self._ctx, C.cast(th, C.c_void_p), sh), "set_kpoint")
+
+    def _cmat(self, t, name: str):
+        torch = _torch()
+        if not (t.is_cuda and t.dtype == torch.complex128 and t.dim() == 2 and t.stride(1) == 1):
+            raise ValueError(f"{name}: need a 2-D complex128 CUDA tensor (ncols, ld) contiguous along ld")
+        if t.shape[1] < self.nd:
+            raise ValueError(f"{name}: ld {t.shape[1]} < N_d {self.nd}")
+        return C.c_void_p(t.data_ptr()), int(t.stride(0)) if t.shape[0] > 1 else int(t.shape[1]), int(t.shape[0])
+
+    def hamiltonian_apply_k(self, X, Y=None):
+        torch = _torch()
+        xp, ldx, ncols = self._cmat(X, "X")
+        if Y is None:
+            Y = torch.empty_like(X)
+        yp, ldy, _ = self._cmat(Y, "Y")
+        ws = self._workspace(OP_HAMILTONIAN_APPLY_K, ncols, 0)
+        _check(self.lib.sparc_gpu_hamiltonian_apply_k(self._ctx, xp, ldx, yp, ldy, ncols, ws, self._stream()), "hamiltonian_apply_k")
+        return Y
+
+    def chebyshev_filter_k(self, Psi, degree: int, a: float, b: float, a0: float, col_block: int = 0):
+        pp, ld, ns = self._cmat(Psi, "Psi")
+        ws = self._workspace(OP_CHEBYSHEV_FILTER_K, ns, col_block)
+        _check(self.lib.sparc_gpu_chebyshev_filter_k(self._ctx, pp, ld, ns, int(degree), float(a), float(b), float(a0),
+                                                     int(col_block), ws, self._stream()), "chebyshev_filter_k")
+        return Psi
+
+    def project_k(self, Psi, col_block: int = 0):
+        torch = _torch()
+        pp, ld, ns = self._cmat(Psi, "Psi")
+        Hs = torch.empty((ns, ns), dtype=torch.complex128, device=Psi.device)
+        Ms = torch.empty_like(Hs)
+        ws = self._workspace(OP_PROJECT_K, ns, col_block)
+        _check(self.lib.sparc_gpu_project_k(self._ctx, pp, ld, ns, C.c_void_p(Hs.data_ptr()), C.c_void_p(Ms.data_ptr()),
+                                            int(col_block), ws, self._stream()), "project_k")
+        return Hs, Ms       # element [j, i] = M_ij (column-major)
+
+    def rotate_k(self, Psi, Q, row_panel: int = 0):
+        torch = _torch()
+        pp, ld, ns = self._cmat(Psi, "Psi")
+        assert Q.is_cuda and Q.dtype == torch.complex128 and Q.shape == (ns, ns) and Q.is_contiguous()
+        ws = self._workspace(OP_ROTATE_K, ns, row_panel)
+        _check(self.lib.sparc_gpu_rotate_k(self._ctx, pp, ld, ns, C.c_void_p(Q.data_ptr()), int(row_panel), ws, self._stream()),
+               "rotate_k")
+        return Psi
 
     def project(self, Psi, col_block: int = 0, Hs=None, Ms=None):
         torch = _torch()

@@ -18,7 +18,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libsparc_gpu.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
-SOURCES = ["context.cu", "stencil_generic.cu", "stencil_tma.cu", "stencil_dmma.cu", "nonlocal.cu", "nonlocal_brick.cu", "gemm.cu", "fill.cu", "peaks.cu", "step_host.cu", "gradient.cu", "eig.cu"]
+SOURCES = ["context.cu", "stencil_generic.cu", "stencil_tma.cu", "stencil_dmma.cu", "nonlocal.cu", "nonlocal_brick.cu", "gemm.cu", "fill.cu", "peaks.cu", "step_host.cu", "gradient.cu", "eig.cu", "kpoint.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xptxas", "-v", "-I", INCLUDE]

@@ -107,6 +107,7 @@ void free_tables(sparc_gpu_ctx *c)
     cudaFree(c->d_cov_ptr); cudaFree(c->d_cov_ent); cudaFree(c->d_veff);
     for (int k = 0; k < 2; ++k) if (c->copy_stream[k]) { cudaStreamDestroy(c->copy_stream[k]); c->copy_stream[k] = nullptr; }
     nlb_free(c);
+    kpoint_free(c);
 }
 
 int validate_desc(const sparc_gpu_desc *d)
@@ -254,6 +255,11 @@ int ws_layout(const sparc_gpu_ctx *c, int op, int64_t ns, int64_t block, WsLayou
         off += round_up_i64(4 * np * np * 8 + 8 * np * 8 + 4096, A);
         break;
     }
+    case SPARC_GPU_OP_HAMILTONIAN_APPLY_K:
+    case SPARC_GPU_OP_CHEBYSHEV_FILTER_K:
+    case SPARC_GPU_OP_PROJECT_K:
+    case SPARC_GPU_OP_ROTATE_K:
+        return ws_layout_k(c, op, ns, block, L);
     case SPARC_GPU_OP_ROTATE: {
         int64_t rp = block > 0 ? block : default_row_panel(c, ns);
         rp = std::min<int64_t>(rp, c->nd);
@@ -402,6 +408,7 @@ int sparc_gpu_create(const sparc_gpu_desc *desc, sparc_gpu_ctx **out)
         }
         c->n_covered = (int64_t)cov_idx.size();
         std::vector<CoverEntry> ent((size_t)c->supp_total);
+        c->h_cov_row.assign((size_t)c->supp_total, 0);
         for (int J = 0; J < na; ++J) {
             const int64_t s0 = desc->supp_ptr[J], nJ = desc->supp_ptr[J + 1] - s0;
             for (int64_t t = 0; t < nJ; ++t) {
@@ -410,6 +417,7 @@ int sparc_gpu_create(const sparc_gpu_desc *desc, sparc_gpu_ctx **out)
                 e.chi_off = desc->chi_ptr[J] + t;
                 e.n_j = (int32_t)nJ;
                 e.pofs_p = (pofs[J] << 8) | desc->n_proj[J];
+                c->h_cov_row[(size_t)slot[(size_t)i]] = s0 + t;
                 ent[(size_t)slot[(size_t)i]++] = e;      // atoms in ascending J order per point: deterministic
             }
         }

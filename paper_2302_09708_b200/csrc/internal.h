@@ -3,6 +3,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <vector>
+
 #include "../../include/sparc_gpu.h"
 
 #define SPARC_MAX_RADIUS 6
@@ -104,6 +106,12 @@ struct sparc_gpu_ctx {
     uint64_t func_attr_done = 0;   // kernel variants whose dynamic shared-memory attribute is set (nonlocal_brick.cu)
     // driver entry point for tensor-map encoding (resolved at create; NULL if unavailable)
     void *fn_encode_tiled = nullptr;
+    // k-point state (kpoint.cu): Bloch phase per axis, exp(i phi_t) per support row and per cover entry
+    double k_theta[3] = {0, 0, 0};
+    int k_set = 0;
+    double2 *d_k_phase = nullptr;        // [supp_total]
+    double2 *d_k_cov_phase = nullptr;    // [supp_total], in the order of d_cov_ent
+    std::vector<int64_t> h_cov_row;      // host: global support row of each cover entry
     // copy streams of the host-buffer entry point (step_host.cu), created on first use
     cudaStream_t copy_stream[2] = {nullptr, nullptr};
     // optional per-kernel CUDA-event timing (option "profile"); NULL when off
@@ -125,7 +133,7 @@ struct DeviceGuard {
 // Kernel kinds for the event profiler and the launch counters.
 enum KernelKind {
     KK_STENCIL_GENERIC = 0, KK_STENCIL_TMA = 1, KK_NL_PROJECT = 2, KK_NL_PULL = 3, KK_GEMM_TN = 4,
-    KK_GEMM_NN = 5, KK_SPLITK_REDUCE = 6, KK_COPY2D = 7, KK_NL_FUSED = 8, KK_NL_BRICK = 9, KK_GRADIENT = 10, KK_EIG = 11, KK_COUNT = 12
+    KK_GEMM_NN = 5, KK_SPLITK_REDUCE = 6, KK_COPY2D = 7, KK_NL_FUSED = 8, KK_NL_BRICK = 9, KK_GRADIENT = 10, KK_EIG = 11, KK_KPOINT = 12, KK_COUNT = 13
 };
 // Bracket one kernel launch with events when profiling is on (no-ops otherwise); both bump the counters.
 void prof_begin(sparc_gpu_ctx *ctx, int kind, cudaStream_t st);
@@ -157,6 +165,8 @@ struct WsLayout {
 };
 int ws_layout(const sparc_gpu_ctx *c, int op, int64_t ns, int64_t block, WsLayout *L);
 int ws_check(const sparc_gpu_ctx *c, const WsLayout &L);
+int ws_layout_k(const sparc_gpu_ctx *c, int op, int64_t ns, int64_t block, WsLayout *L);   // k-point operators (kpoint.cu)
+void kpoint_free(sparc_gpu_ctx *c);
 
 // ---- kernel launchers (each returns a sparc_gpu_status and bumps ctx->kernel_launches) ----------
 
