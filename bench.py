@@ -12,9 +12,10 @@ largest one, 81.5 GB of Psi on one GPU); the default run then also times configs
 33) workload for a few steps each and reports them under `per_config`.  `e2e` is the whole step through the host-buffer
 entry point sparc_gpu_chefsi_step_host.
 
-N > 1: the path shards by orbital columns with no data-path collective for the filter (PAPER.md:120, 190);
-this build runs N independent replicas of the workload ("replicas only") and reports
-the aggregate, scaling = "weak".
+N > 1 (one rank per GPU under torchrun; `python bench.py --gpus N` starts the ranks itself): --parallelism shard (default)
+partitions ONE workload as the paper does -- filter by columns without communication, all-to-all,
+projection / rotation by rows with an all-reduce of Hs, Ms (paper_2302_09708_b200/dist.py) -- scaling = "strong";
+--parallelism replicas runs N independent copies, scaling = "weak".
 
 --impl reference times the CPU oracle (oracle/, acc_t = double build) on the host cores: a deliberately slow
 program, reported as context.
@@ -447,6 +448,91 @@ def bench_config(env, config, steps, warmup, *, col_block=0, stencil_path=0, ste
     return res
 
 
+def bench_shard(env, config, steps, warmup, col_block=0):
+    """N > 1: ONE workload partitioned over the ranks as the paper does (dist.py): columns for the
+    filter, rows for projection / rotation, an all-to-all each way and an all-reduce of Hs / Ms.  Strong scaling."""
+    torch, dist, api, wlmod = env["torch"], env["dist"], env["api"], env["wlmod"]
+    world, rank, local_rank, dev = env["world"], env["rank"], env["local_rank"], env["dev"]
+    from paper_2302_09708_b200 import dist as pdist
+
+    wl = wlmod.make_workload(config)
+    g = api.SparcGpu(wl, device=local_rank)
+    local = pdist.SparcGpuLocal(g)
+    nd, ns, m = wl.nd, wl.ns, wl.degree
+    cb, ce = pdist.partition(ns, world, rank)
+    Xc = torch.empty((ce - cb, nd), dtype=torch.float64, device=dev)
+
+    def refill():       # this rank's columns of the same global seeded block
+        if ce > cb:
+            api.fill_uniform(Xc, wl.seed, wlmod.STREAM_PSI, cb * nd, -1.0, 1.0)
+    Q = api.colmajor_from_numpy(wl.q_matrix(), device=dev)
+    col_block = col_block if col_block else (wl.col_block or 1024)
+    names = ["start", "filter", "to_rows", "project", "solve", "rotate", "to_columns"]
+
+    def one_step(record=None):
+        refill()
+        evs = {}
+
+        def mark(name):
+            if record is not None:
+                e = torch.cuda.Event(enable_timing=True)
+                e.record()
+                evs[name] = e
+        pdist.chefsi_step(local, Xc, nd, ns, m, wl.a, wl.b, wl.a0, Q=Q, col_block=col_block, timers={"mark": mark})
+        if record is not None:
+            record.append(evs)
+
+    for _ in range(warmup):
+        one_step()
+    pdist.barrier(dev)
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    launches0 = g.get_info("kernel_launches")
+    rec = []
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        one_step(rec)
+    pdist.barrier(dev)
+    t_wall = time.perf_counter() - t0
+    launches = g.get_info("kernel_launches") - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    phase = [sum(e[names[i]].elapsed_time(e[names[i + 1]]) for e in rec) / steps for i in range(len(names) - 1)]
+    phase = pdist.max_over_ranks(phase, dev)                     # slowest rank per phase
+    filt = phase[0]
+    step_ms = sum(phase)
+    # end to end: this rank's columns from pinned host memory and back around the same step
+    host = torch.empty((ce - cb, nd), dtype=torch.float64, pin_memory=True)
+    refill()
+    host.copy_(Xc)
+    pdist.barrier(dev)
+    t0 = time.perf_counter()
+    Xc.copy_(host, non_blocking=True)
+    pdist.chefsi_step(local, Xc, nd, ns, m, wl.a, wl.b, wl.a0, Q=Q, col_block=col_block)
+    host.copy_(Xc, non_blocking=True)
+    pdist.barrier(dev)
+    e2e_s = pdist.max_over_ranks([time.perf_counter() - t0], dev)[0]
+    units = float(nd) * ns * m
+    res = {
+        "value": units / (filt * 1e-3), "ms_per_step": step_ms, "scaling": "strong",
+        "config": {"workload": wl.name, "grid": list(wl.n), "nd": nd, "ns": ns, "degree": m, "atoms": wl.n_atoms,
+                   "col_block": col_block, "stencil_path": g.get_info("stencil_path_last"),
+                   "parallelism": f"shard x{world}: filter by columns, all-to-all, project / rotate by rows, all-reduce of Hs, Ms "
+                                  "(NCCL)",
+                   "l2": "each rank's slice is larger than the 126 MB L2 and is regenerated between steps"},
+        "hbm_gbs": units / (filt * 1e-3) * ALG_BYTES_PER_UNIT / 1e9,
+        "subspace_tflops": 3 * 2.0 * nd * ns * ns / ((phase[2] + phase[4]) * 1e-3) / 1e12,
+        "step_ms": dict(zip(["filter", "to_rows", "project", "solve", "rotate", "to_columns"], phase),
+                        wall_per_step=t_wall / steps * 1e3),
+        "steps": steps, "warmup": warmup, "clocks": clocks,
+        "e2e": {"value": units / e2e_s, "unit": UNIT, "h2d_bytes_per_step": ns * nd * 8, "d2h_bytes_per_step": ns * nd * 8,
+                "step_s": e2e_s, "what": "every rank: its columns pinned host -> device, the distributed step, device -> host"},
+        "gpu_launches": int(launches), "roofline": None, "roofline_by_kernel": {}, "filter_roofs": None, "cpu_baseline": None,
+    }
+    g.close()
+    return res
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -465,9 +551,12 @@ def run_ours(args):
     env = {"torch": torch, "dist": dist, "api": api, "wlmod": wlmod, "world": world, "rank": rank,
            "local_rank": local_rank, "dev": dev}
 
-    res = bench_config(env, args.config, args.steps, args.warmup, col_block=args.col_block,
-                       stencil_path=args.stencil_path, stencil_stages=args.stencil_stages,
-                       do_e2e=not args.no_e2e, do_cpu=not args.no_cpu)
+    if (world > 1 or args.force_shard) and args.parallelism == "shard":
+        res = bench_shard(env, args.config, args.steps, args.warmup, col_block=args.col_block)
+    else:
+        res = bench_config(env, args.config, args.steps, args.warmup, col_block=args.col_block,
+                           stencil_path=args.stencil_path, stencil_stages=args.stencil_stages,
+                           do_e2e=not args.no_e2e, do_cpu=not args.no_cpu)
     # the other workloads of BASELINE.json (and the sixth, finer-mesh one), a few steps each, same measurement
     per_config = {}
     if args.per_config and world == 1:
@@ -484,7 +573,8 @@ def run_ours(args):
     if rank == 0:
         line = {
             "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": res["ms_per_step"], "higher_is_better": True,
+            "scaling": res.get("scaling", "weak"),
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": res["config"],
             "hbm_gbs": res["hbm_gbs"],
@@ -521,6 +611,10 @@ def main():
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiling runs)")
     ap.add_argument("--per-config", type=int, default=-1,
                     help="1: after the headline workload also time the other workloads (per_config key); default: on for the default workload")
+    ap.add_argument("--parallelism", default="shard", choices=["shard", "replicas"],
+                    help="N > 1: 'shard' partitions ONE workload over the ranks as the paper does (strong scaling); "
+                         "'replicas' runs N independent copies (weak scaling)")
+    ap.add_argument("--force-shard", action="store_true", help="take the shard code path with one rank too (testing)")
     ap.add_argument("--stencil-path", type=int, default=0, help="0 library default, 2 TMA + DFMA kernel, 3 TMA + DMMA hybrid")
     ap.add_argument("--stencil-stages", type=int, default=0, help="TMA ring depth (0 = library default)")
     args = ap.parse_args()
@@ -528,6 +622,16 @@ def main():
         args.per_config = 1 if args.config == 4 else 0
     if args.impl == "reference":
         return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # plain `python bench.py --gpus N`: start the N ranks ourselves, exactly as the driver would
+        import socket
+        sk = socket.socket()
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+        sk.close()
+        os.execv(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+                                  "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)]
+                 + sys.argv[1:])
     return run_ours(args)
 
 

@@ -71,7 +71,8 @@ typedef enum {
     SPARC_GPU_OP_HAMILTONIAN_APPLY_K = 7,
     SPARC_GPU_OP_CHEBYSHEV_FILTER_K = 8,
     SPARC_GPU_OP_PROJECT_K = 9,
-    SPARC_GPU_OP_ROTATE_K = 10
+    SPARC_GPU_OP_ROTATE_K = 10,
+    SPARC_GPU_OP_GRAM = 11
 } sparc_gpu_op;
 
 /* Problem description (all pointers HOST, copied at create).  PAPER.md:118 "The matrix X, effective
@@ -199,6 +200,21 @@ int sparc_gpu_project_k(sparc_gpu_ctx *ctx, const double *Psi_dev, int64_t ld, i
 /* Psi <- Psi Q in place by row panels, Q complex ns x ns (PAPER.md:166 cublasZgemm). */
 int sparc_gpu_rotate_k(sparc_gpu_ctx *ctx, double *Psi_dev, int64_t ld, int64_t ns, const double *Q_dev, int64_t row_panel,
                        void *ws_dev, void *stream);
+
+/* ---- local pieces of the row-partitioned projection and rotation -----------------------------
+ * With X and Y = H X redistributed into row blocks X~^(k), Y~^(k) (eq. 5), rank k forms
+ * H~^(k) = X~^(k)T Y~^(k), M~^(k) = X~^(k)T X~^(k) (eqs. 6-8; the sums over k are one all-reduce each, made by the
+ * caller, paper_2302_09708_b200/dist.py) and later rotates its rows, X^(k) = X~^(k) Z~ (eqs. 10-11). */
+
+/* C (m x n, column-major, ld = m) = A^T B, contraction over `nrows` rows; A: nrows x m (lda), B: nrows x n (ldb).
+ * symmetric != 0 (needs m = n and a product that IS symmetric, e.g. A = B): upper-triangle tiles + mirror (R12).
+ * Workspace op GRAM with ns = max(m, n). */
+int sparc_gpu_gram(sparc_gpu_ctx *ctx, const double *A_dev, int64_t lda, const double *B_dev, int64_t ldb, int64_t nrows,
+                   int64_t m, int64_t n, double *C_dev, int symmetric, void *ws_dev, void *stream);
+
+/* X <- X Q in place on a block of `nrows` rows (ld >= nrows): sparc_gpu_rotate for a row block (workspace op ROTATE). */
+int sparc_gpu_rotate_rows(sparc_gpu_ctx *ctx, double *X_dev, int64_t ld, int64_t nrows, int64_t ns, const double *Q_dev,
+                          int64_t row_panel, void *ws_dev, void *stream);
 
 /* One whole CheFSI step -- filter, project, rotate -- for a block that lives in HOST memory (what the paper's code does
  * around every step with cublasSet/GetVector: PAPER.md:118, 128, 138, 146, 158, 166), with the PCIe copies overlapped with

@@ -23,6 +23,7 @@ _lib = None
 OP_HAMILTONIAN_APPLY, OP_CHEBYSHEV_FILTER, OP_PROJECT, OP_ROTATE = 0, 1, 2, 3
 OP_GRADIENT_PROJECT, OP_NONLOCAL_FORCE, OP_EIGENSOLVE = 4, 5, 6
 OP_HAMILTONIAN_APPLY_K, OP_CHEBYSHEV_FILTER_K, OP_PROJECT_K, OP_ROTATE_K = 7, 8, 9, 10
+OP_GRAM = 11
 
 EXPORTS = ["sparc_gpu_create", "sparc_gpu_destroy", "sparc_gpu_set_veff", "sparc_gpu_workspace_bytes",
            "sparc_gpu_set_workspace_size",
@@ -30,7 +31,7 @@ EXPORTS = ["sparc_gpu_create", "sparc_gpu_destroy", "sparc_gpu_set_veff", "sparc
            "sparc_gpu_rotate", "sparc_gpu_chefsi_step_host", "sparc_gpu_gradient",
            "sparc_gpu_nl_project", "sparc_gpu_gradient_project", "sparc_gpu_nonlocal_force", "sparc_gpu_eigensolve", "sparc_gpu_set_kpoint",
            "sparc_gpu_hamiltonian_apply_k", "sparc_gpu_chebyshev_filter_k", "sparc_gpu_project_k", "sparc_gpu_rotate_k",
-           "sparc_gpu_fill_uniform", "sparc_gpu_set_option", "sparc_gpu_get_info", "sparc_gpu_probe_peak",
+           "sparc_gpu_gram", "sparc_gpu_rotate_rows", "sparc_gpu_fill_uniform", "sparc_gpu_set_option", "sparc_gpu_get_info", "sparc_gpu_probe_peak",
            "sparc_gpu_error_string", "sparc_gpu_version"]
 
 
@@ -81,6 +82,8 @@ def load_library(build_if_missing: bool = True):
     lib.sparc_gpu_chebyshev_filter_k.argtypes = [P, P, I64, I64, I, D, D, D, I64, P, P]
     lib.sparc_gpu_project_k.argtypes = [P, P, I64, I64, P, P, I64, P, P]
     lib.sparc_gpu_rotate_k.argtypes = [P, P, I64, I64, P, I64, P, P]
+    lib.sparc_gpu_gram.argtypes = [P, P, I64, P, I64, I64, I64, I64, P, I, P, P]
+    lib.sparc_gpu_rotate_rows.argtypes = [P, P, I64, I64, I64, P, I64, P, P]
     lib.sparc_gpu_fill_uniform.argtypes = [P, I64, C.c_uint64, C.c_uint64, C.c_uint64, D, D, I, P]
     lib.sparc_gpu_probe_peak.argtypes = [I, I, C.POINTER(D), P, I64, P]
     lib.sparc_gpu_set_option.argtypes = [P, C.c_char_p, I64]
@@ -445,6 +448,26 @@ class SparcGpu:
         _check(self.lib.sparc_gpu_rotate_k(self._ctx, pp, ld, ns, C.c_void_p(Q.data_ptr()), int(row_panel), ws, self._stream()),
                "rotate_k")
         return Psi
+
+    # ---- NEXT-2: local pieces of the row-partitioned projection / rotation (matrices (ncols, ld) with ld >= nrows) ------
+    def gram(self, A, B, nrows: int, symmetric: bool = False, out=None):
+        torch = _torch()
+        m, n = int(A.shape[0]), int(B.shape[0])
+        lda = int(A.stride(0)) if m > 1 else int(A.shape[1])
+        ldb = int(B.stride(0)) if n > 1 else int(B.shape[1])
+        Cm = out if out is not None else torch.empty((n, m), dtype=torch.float64, device=A.device)
+        ws = self._workspace(OP_GRAM, max(m, n), 0)
+        _check(self.lib.sparc_gpu_gram(self._ctx, C.c_void_p(A.data_ptr()), lda, C.c_void_p(B.data_ptr()), ldb, int(nrows), m, n,
+                                       C.c_void_p(Cm.data_ptr()), 1 if symmetric else 0, ws, self._stream()), "gram")
+        return Cm           # (n, m) tensor holding the column-major m x n matrix
+
+    def rotate_rows(self, X, nrows: int, Q, row_panel: int = 0):
+        ns = int(X.shape[0])
+        ld = int(X.stride(0)) if ns > 1 else int(X.shape[1])
+        ws = self._workspace(OP_ROTATE, ns, row_panel)
+        _check(self.lib.sparc_gpu_rotate_rows(self._ctx, C.c_void_p(X.data_ptr()), ld, int(nrows), ns, C.c_void_p(Q.data_ptr()),
+                                              int(row_panel), ws, self._stream()), "rotate_rows")
+        return X
 
     def project(self, Psi, col_block: int = 0, Hs=None, Ms=None):
         torch = _torch()

@@ -260,6 +260,12 @@ int ws_layout(const sparc_gpu_ctx *c, int op, int64_t ns, int64_t block, WsLayou
     case SPARC_GPU_OP_PROJECT_K:
     case SPARC_GPU_OP_ROTATE_K:
         return ws_layout_k(c, op, ns, block, L);
+    case SPARC_GPU_OP_GRAM: {
+        const int64_t n = std::max<int64_t>(ns, 1);
+        L->block = n; L->ldw = n; L->off_w = off; L->off_g = off;
+        off += round_up_i64(gemm_tn_ws_bytes(c, n, n, c->nd), A);
+        break;
+    }
     case SPARC_GPU_OP_ROTATE: {
         int64_t rp = block > 0 ? block : default_row_panel(c, ns);
         rp = std::min<int64_t>(rp, c->nd);
@@ -642,6 +648,44 @@ int sparc_gpu_rotate(sparc_gpu_ctx *ctx, double *Psi, int64_t ld, int64_t ns, co
     for (int64_t r0 = 0; r0 < ctx->nd; r0 += L.block) {
         const int64_t nr = std::min(L.block, ctx->nd - r0);
         SPARC_TRY(rotate_panel(ctx, Psi + r0, ld, nr, ns, Q, T, L.ldw, st));
+    }
+    return SPARC_GPU_SUCCESS;
+}
+
+// ---- building blocks of the row-partitioned (multi-GPU) projection and rotation, SURVEY.md section 8(f) NEXT-2 -------------
+
+int sparc_gpu_gram(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const double *B, int64_t ldb, int64_t nrows, int64_t m,
+                   int64_t n, double *C, int symmetric, void *ws, void *stream)
+{
+    if (!ctx || nrows < 0 || m < 0 || n < 0) return SPARC_GPU_INVALID_ARG;
+    if (m == 0 || n == 0) return SPARC_GPU_SUCCESS;
+    if (!A || !B || !C || !ws || lda < nrows || ldb < nrows || (symmetric && m != n)) return SPARC_GPU_INVALID_ARG;
+    DeviceGuard dg(ctx->device);
+    if (!dg.ok) return SPARC_GPU_CUDA_ERROR;
+    cudaStream_t st = (cudaStream_t)stream;
+    WsLayout L;
+    SPARC_TRY(ws_layout(ctx, SPARC_GPU_OP_GRAM, std::max(m, n), 0, &L));
+    SPARC_TRY(ws_check(ctx, L));
+    if (nrows == 0) { SPARC_CUDA_TRY(cudaMemsetAsync(C, 0, (size_t)m * n * 8, st)); return SPARC_GPU_SUCCESS; }
+    const bool sym = symmetric && ctx->opt_gemm_full == 0;
+    SPARC_TRY(launch_gemm_tn(ctx, A, lda, B, ldb, C, m, m, n, nrows, (char *)ws + L.off_g, sym ? 0 : -1, st));
+    if (sym) SPARC_TRY(launch_mirror_upper(ctx, C, m, m, st));
+    return SPARC_GPU_SUCCESS;
+}
+
+int sparc_gpu_rotate_rows(sparc_gpu_ctx *ctx, double *X, int64_t ld, int64_t nrows, int64_t ns, const double *Q,
+                          int64_t row_panel, void *ws, void *stream)
+{
+    if (!ctx || ns < 0 || nrows < 0) return SPARC_GPU_INVALID_ARG;
+    if (ns == 0 || nrows == 0) return SPARC_GPU_SUCCESS;
+    if (!X || !Q || !ws || ld < nrows) return SPARC_GPU_INVALID_ARG;
+    DeviceGuard dg(ctx->device);
+    if (!dg.ok) return SPARC_GPU_CUDA_ERROR;
+    int64_t rp = 0, ldw = 0;
+    SPARC_TRY(rotate_layout(ctx, ns, row_panel, &rp, &ldw));
+    for (int64_t r0 = 0; r0 < nrows; r0 += rp) {
+        const int64_t nr = std::min(rp, nrows - r0);
+        SPARC_TRY(rotate_panel(ctx, X + r0, ld, nr, ns, Q, (double *)ws, ldw, (cudaStream_t)stream));
     }
     return SPARC_GPU_SUCCESS;
 }

@@ -1,5 +1,7 @@
-"""Host logic of the N > 1 launch (paper_2302_09708_b200/dist.py) on CPU: the paper's column / row partition
- and the max-over-ranks reduction, with two gloo processes."""
+"""The N > 1 data path (paper_2302_09708_b200/dist.py) on CPU with two gloo processes: the paper's column / row partitions
+(PAPER.md:104-108), the column <-> row redistributions, the all-reduce of the partial subspace
+matrices and the whole distributed step, with the local kernels replaced by the oracle (the CUDA kernels
+need a GPU; tests may call oracle/) and the result compared with the single-process oracle."""
 import os
 import socket
 
@@ -43,6 +45,54 @@ def _free_port():
     return port
 
 
+class OracleLocal:
+    """Stand-in for the CUDA kernels in the CPU test: the same five local operations, computed by the oracle."""
+
+    def __init__(self, wl):
+        from oracle import oracle as orc
+        self.orc = orc
+        self.H = orc.Hamiltonian(wl)
+        self.nd = wl.nd
+
+    def _np(self, X, rows):
+        return np.asfortranarray(X[:, :rows].numpy().T)
+
+    def filter(self, X, degree, a, b, a0, col_block=0):
+        import torch
+        F = self.H.chebyshev_filter(self._np(X, self.nd), degree, a, b, a0)
+        X[:, :self.nd] = torch.from_numpy(np.ascontiguousarray(F.T))
+        return X
+
+    def apply(self, X):
+        import torch
+        Y = torch.zeros_like(X)
+        Y[:, :self.nd] = torch.from_numpy(np.ascontiguousarray(self.H.apply(self._np(X, self.nd)).T))
+        return Y
+
+    def gram(self, A, B, nrows, symmetric):
+        import torch
+        G = self.orc.gram(self._np(A, nrows), self._np(B, nrows)) if nrows > 0 else np.zeros((A.shape[0], B.shape[0]))
+        return torch.from_numpy(np.ascontiguousarray(G.T))
+
+    def rotate_rows(self, X, nrows, Q):
+        import torch
+        if nrows > 0:
+            R = self.orc.rotate(self._np(X, nrows), np.asfortranarray(Q.numpy().T))
+            X[:, :nrows] = torch.from_numpy(np.ascontiguousarray(R.T))
+        return X
+
+    def eigensolve(self, Hs, Ms):
+        import torch
+        D, Z = self.orc.sygv(np.asfortranarray(Hs.numpy().T), np.asfortranarray(Ms.numpy().T))
+        return torch.from_numpy(D), torch.from_numpy(np.ascontiguousarray(Z.T))
+
+
+def _make_wl():
+    from paper_2302_09708_b200 import workloads as wlmod
+    pos = np.array([[1.0, 2.0, 3.0], [4.5, 5.0, 0.4]])
+    return wlmod.make_custom("dist", (13, 15, 15), (0.5, 0.45, 0.4), (0, 0, 1), 7, 4, pos, [4, 9], 2.3, seed=51)
+
+
 def _worker(rank, world, port, out):
     import torch
     import torch.distributed as dist
@@ -50,35 +100,81 @@ def _worker(rank, world, port, out):
     os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
-        # each rank "filters" its column slice of a shared synthetic block: disjoint slices that tile the block
-        ns = 37
-        b, e = pdist.partition(ns, world, rank)
-        mine = torch.zeros(ns, dtype=torch.float64)
-        mine[b:e] = 1.0
-        dist.all_reduce(mine)
-        covered = bool(torch.equal(mine, torch.ones(ns, dtype=torch.float64)))
+        # reductions used by bench.py
         times = pdist.max_over_ranks([1.0 + rank, 5.0 - rank])
-        units = pdist.sum_over_ranks([float(e - b)])
+        units = pdist.sum_over_ranks([3.0 + rank])
+        # redistribution round trip on a labelled block: element (i, j) = i + 10000 j
+        nd, ns = 37, 5
+        cb, ce = pdist.partition(ns, world, rank)
+        rb, re_ = pdist.partition(nd, world, rank)
+        full = (np.arange(nd)[:, None] + 10000.0 * np.arange(ns)[None, :])
+        Xc = torch.zeros((ce - cb, nd + 3), dtype=torch.float64)
+        Xc[:, :nd] = torch.from_numpy(np.ascontiguousarray(full[:, cb:ce].T))
+        Xr = pdist.columns_to_rows(Xc, nd, ns, col_block=2)      # blocks with a ragged tail: the ranks own 3 and 2 columns
+        rows_ok = bool(np.array_equal(Xr.numpy().T, full[rb:re_, :]))
+        back = torch.zeros_like(Xc)
+        pdist.rows_to_columns(Xr, nd, ns, out=back, col_block=2)
+        round_ok = bool(torch.equal(back, Xc))
+        # the whole step, caller's Q and device-side solve
+        wl = _make_wl()
+        local = OracleLocal(wl)
+        cb, ce = pdist.partition(wl.ns, world, rank)
+        X = wl.psi_columns(range(wl.ns))
+        rng = np.random.default_rng(5)
+        Q = np.linalg.qr(rng.standard_normal((wl.ns, wl.ns)))[0]
+        res = {}
+        for mode in ("given_q", "solve"):
+            Xc = torch.from_numpy(np.ascontiguousarray(X[:, cb:ce].T)).clone()
+            Qt = torch.from_numpy(np.ascontiguousarray(Q.T)) if mode == "given_q" else None
+            Hs, Ms, D = pdist.chefsi_step(local, Xc, wl.nd, wl.ns, wl.degree, wl.a, wl.b, wl.a0, Q=Qt,
+                                            col_block=0 if mode == "given_q" else 3)
+            res[mode] = (Xc.numpy().T.copy(), Hs.numpy().T.copy(), Ms.numpy().T.copy(), None if D is None else D.numpy().copy())
         pdist.barrier()
-        out.put((rank, covered, times, units))
+        out.put((rank, times, units, rows_ok, round_ok, (cb, ce), res))
     finally:
         dist.destroy_process_group()
 
 
-def test_two_rank_gloo_reduction():
+def test_two_rank_gloo_step_matches_single_process_oracle():
     import torch.multiprocessing as mp
+    from oracle import oracle as orc
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
     port = _free_port()
     procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
     for p in procs:
         p.start()
-    res = sorted(q.get(timeout=120) for _ in procs)
+    res = sorted((q.get(timeout=300) for _ in procs), key=lambda t: t[0])
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
-    for rank, covered, times, units in res:
-        assert covered
+    for rank, times, units, rows_ok, round_ok, _, _ in res:
         assert times == [2.0, 5.0]           # max over ranks of [1, 5] and [2, 4]
-        assert units == [37.0]
-    assert np.isfinite(res[0][2]).all()
+        assert units == [7.0]
+        assert rows_ok and round_ok
+    # single-process reference: filter -> project -> (Q | solve) -> rotate
+    wl = _make_wl()
+    H = orc.Hamiltonian(wl)
+    X = wl.psi_columns(range(wl.ns))
+    F = H.chebyshev_filter(X, wl.degree, wl.a, wl.b, wl.a0)
+    Hs_o, Ms_o = H.project(F)
+    rng = np.random.default_rng(5)
+    Q = np.linalg.qr(rng.standard_normal((wl.ns, wl.ns)))[0]
+    R_given = orc.rotate(F, Q)
+    D_o, Z_o = orc.sygv(0.5 * (Hs_o + Hs_o.T), Ms_o)
+    for mode in ("given_q", "solve"):
+        got = np.concatenate([r[6][mode][0] for r in res], axis=1)        # columns of rank 0, then rank 1
+        for r in res:
+            Hs, Ms = r[6][mode][1], r[6][mode][2]
+            assert np.linalg.norm(Hs - Hs_o) <= 1e-12 * np.linalg.norm(Hs_o)
+            assert np.linalg.norm(Ms - Ms_o) <= 1e-12 * np.linalg.norm(Ms_o)
+        assert np.array_equal(res[0][6][mode][1], res[1][6][mode][1])    # the all-reduced matrices are the same on both ranks
+        if mode == "given_q":
+            assert np.linalg.norm(got - R_given) <= 1e-12 * np.linalg.norm(R_given)
+        else:
+            D = res[0][6][mode][3]
+            assert np.max(np.abs(D - D_o)) <= 1e-10 * max(1.0, np.abs(D_o).max())
+            # rotated block: M-orthonormal Ritz vectors with Rayleigh quotients D
+            Hs2, Ms2 = H.project(got)
+            assert np.max(np.abs(Ms2 - np.eye(wl.ns))) <= 1e-9
+            assert np.max(np.abs(Hs2 - np.diag(D))) <= 1e-9 * max(1.0, np.abs(D).max())
