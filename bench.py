@@ -533,6 +533,92 @@ def bench_shard(env, config, steps, warmup, col_block=0):
     return res
 
 
+def bench_next_rows(env, config=2):
+    """The SURVEY.md section 8(f) rows measured on one workload's grid and atoms (device-resident inputs, CUDA events, best of
+    3 after a warm-up): gradient stencil, chi^T X, nonlocal force (NEXT-3); device eigensolve (NEXT-1); complex k-point
+    filter / project / rotate (NEXT-4).  NEXT-2 is what `--gpus N` times."""
+    torch, api, wlmod, dev, local_rank = env["torch"], env["api"], env["wlmod"], env["dev"], env["local_rank"]
+    wl = wlmod.make_workload(config)
+    g = api.SparcGpu(wl, device=local_rank)
+    nd, ns = wl.nd, min(wl.ns, 1024)
+    hbm_peak, hbm_src = measured_peaks()
+    dmma_peak = env["peaks"][1] if "peaks" in env else api.probe_peak(1, local_rank)
+    out = {"workload": wl.name, "columns": ns, "peaks": {"hbm_gbs": hbm_peak, "hbm_source": hbm_src, "dmma_tflops": dmma_peak}}
+
+    def timed(fn, reps=3):
+        fn()
+        torch.cuda.synchronize()
+        best = None
+        for _ in range(reps):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fn()
+            b.record()
+            torch.cuda.synchronize()
+            ms = a.elapsed_time(b)
+            best = ms if best is None else min(best, ms)
+        return best
+
+    psi = torch.empty((ns, nd), dtype=torch.float64, device=dev)
+    api.fill_uniform(psi, wl.seed, wlmod.STREAM_PSI, 0, -1.0, 1.0)
+    Y = torch.empty_like(psi)
+    supp_rows = float(wl.supp_idx.shape[0])
+    pbar = float(wl.chi.shape[0]) / max(supp_rows, 1.0)
+    grad = {}
+    for axis in range(3):
+        ms = timed(lambda: g.gradient(psi, axis, Y))
+        gbs = 16.0 * nd * ns / (ms * 1e-3) / 1e9
+        grad["xyz"[axis]] = {"ms": ms, "achieved": gbs, "unit": "GB/s", "peak": hbm_peak, "frac": gbs / hbm_peak, "bound": "hbm",
+                             "alg_bytes_per_point": 16}
+    out["gradient"] = grad
+    ms = timed(lambda: g.nl_project(psi))
+    out["nl_project"] = {"ms": ms, "achieved": 2.0 * supp_rows * pbar * ns / (ms * 1e-3) / 1e12, "unit": "TFLOP/s",
+                         "note": "chi^T X, 2 flop per (support row, projector, column); per-atom FMA kernel"}
+    occ = torch.from_numpy(wl.occupations()[:ns].copy()).to(dev)
+    ms = timed(lambda: g.nonlocal_force(psi, occ))
+    out["nonlocal_force"] = {"ms": ms, "orbitals_per_s": ns / (ms * 1e-3),
+                             "what": "3 gradient passes + 4 projector contractions + the force contraction per column block"}
+    del Y
+    # NEXT-1: device eigensolve on a well-conditioned synthetic pencil of the subspace sizes of configs 1-2 (and 2048)
+    eig = {}
+    for n in (256, 1024, 2048):
+        A = torch.empty((n, n), dtype=torch.float64, device=dev)
+        api.fill_uniform(A, 77, 1, 0, -1.0, 1.0)
+        Hs = (A + A.T).contiguous()
+        Ms = (A @ A.T / n + torch.eye(n, dtype=torch.float64, device=dev)).contiguous()     # SPD input for the timing (torch: input generation only)
+        info = []
+        ms = timed(lambda: info.append(g.eigensolve(Hs, Ms)[2]), reps=2)
+        st = info[-1].cpu().numpy()
+        eig[str(n)] = {"ms": ms, "sweeps": int(st[1]), "status": int(st[0])}
+        del A, Hs, Ms
+    out["eigensolve"] = eig
+    # NEXT-4: complex k-point operators, 256 complex orbitals
+    nk = min(256, ns)
+    g.set_kpoint((0.5 * np.pi, 0.5 * np.pi, 0.0 if wl.bc[2] else 0.5 * np.pi), wl.supp_shift)
+    pk = torch.empty((nk, nd), dtype=torch.complex128, device=dev)
+    api.fill_uniform(torch.view_as_real(pk), wl.seed, wlmod.STREAM_PSI, 0, -1.0, 1.0)
+    m = wl.degree
+    ms = timed(lambda: g.chebyshev_filter_k(pk, m, wl.a, wl.b, wl.a0), reps=2)
+    units = float(nd) * nk * m
+    out["kpoint_filter"] = {"ms": ms, "value": units / (ms * 1e-3), "unit": UNIT + " (complex orbitals)",
+                            "achieved": 48.0 * units / (ms * 1e-3) / 1e9, "peak": hbm_peak, "frac": 48.0 * units / (ms * 1e-3) / 1e9 / hbm_peak,
+                            "bound": "hbm", "alg_bytes_per_unit": 48,
+                            "note": "generic one-thread-per-point complex stencil + per-atom phased projectors (first version)"}
+    api.fill_uniform(torch.view_as_real(pk), wl.seed, wlmod.STREAM_PSI, 0, -1.0, 1.0)
+    ms = timed(lambda: g.project_k(pk), reps=2)
+    out["kpoint_project"] = {"ms": ms, "gemm_tflops_nominal": 2 * 8.0 * nd * nk * nk / (ms * 1e-3) / 1e12, "peak": dmma_peak,
+                             "note": "Hs, Ms = 2 Hermitian products = 4 real TN GEMMs over 2 N_d rows (8 N_d N_s^2 flop each product) "
+                                     "+ H(k) Psi; time includes the H(k) apply"}
+    Qk = torch.linalg.qr(torch.randn(nk, nk, dtype=torch.complex128, device=dev))[0].contiguous()
+    ms = timed(lambda: g.rotate_k(pk, Qk), reps=2)
+    out["kpoint_rotate"] = {"ms": ms, "achieved": 8.0 * nd * nk * nk / (ms * 1e-3) / 1e12, "unit": "TFLOP/s", "peak": dmma_peak,
+                            "frac": 8.0 * nd * nk * nk / (ms * 1e-3) / 1e12 / dmma_peak, "bound": "tensor"}
+    g.close()
+    del psi, pk
+    torch.cuda.empty_cache()
+    return out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -570,6 +656,9 @@ def run_ours(args):
             per_config[str(c)] = {k: r[k] for k in ("value", "hbm_gbs", "subspace_tflops", "ms_per_step", "step_ms", "steps",
                                                      "warmup", "config", "filter_roofs", "roofline_by_kernel", "clocks", "e2e")}
 
+    next_rows = None
+    if args.next_rows and world == 1:
+        next_rows = bench_next_rows(env, 2)
     if rank == 0:
         line = {
             "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -593,6 +682,8 @@ def run_ours(args):
         }
         if per_config:
             line["per_config"] = per_config
+        if next_rows:
+            line["next_rows"] = next_rows
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -611,6 +702,9 @@ def main():
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiling runs)")
     ap.add_argument("--per-config", type=int, default=-1,
                     help="1: after the headline workload also time the other workloads (per_config key); default: on for the default workload")
+    ap.add_argument("--next-rows", type=int, default=-1,
+                    help="1: also time the SURVEY 8(f) rows (gradient / force, eigensolve, k-point operators) under `next_rows`; "
+                         "default: on for the default workload")
     ap.add_argument("--parallelism", default="shard", choices=["shard", "replicas"],
                     help="N > 1: 'shard' partitions ONE workload over the ranks as the paper does (strong scaling); "
                          "'replicas' runs N independent copies (weak scaling)")
@@ -620,6 +714,8 @@ def main():
     args = ap.parse_args()
     if args.per_config < 0:
         args.per_config = 1 if args.config == 4 else 0
+    if args.next_rows < 0:
+        args.next_rows = 1 if args.config == 4 else 0
     if args.impl == "reference":
         return run_reference(args)
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
