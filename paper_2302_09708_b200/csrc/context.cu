@@ -189,8 +189,8 @@ int h_apply_block(sparc_gpu_ctx *c, const double *X, int64_t ldx, double *Y, int
 {
     const int mode = effective_nl_mode(c, X, ldx, Y, ldy);
     if (mode == 3) {      // chi^T X first (X may not be read after Y is written when they alias; they never do here)
-        SPARC_CUDA_TRY(cudaMemsetAsync(D, 0, (size_t)c->n_proj_total * nlb_c_cols(ncols) * 8, st));
-        SPARC_TRY(launch_nl_brick(c, 1, const_cast<double *>(X), ldx, ncols, 0.0, nullptr, D, st));
+        SPARC_CUDA_TRY(cudaMemsetAsync(D, 0, (size_t)nlb_c_doubles(c, ncols) * 8, st));
+        SPARC_TRY(launch_nl_brick(c, 1, const_cast<double *>(X), ldx, ncols, 1.0, nullptr, D, st));
     }
     SPARC_TRY(local_pass(c, X, ldx, Y, ldy, nullptr, 0, ncols, 1.0, 0.0, 0.0, st));
     if (mode == 3) SPARC_TRY(launch_nl_brick(c, 2, Y, ldy, ncols, 1.0, D, nullptr, st));
@@ -227,7 +227,7 @@ int ws_layout(const sparc_gpu_ctx *c, int op, int64_t ns, int64_t block, WsLayou
         L->off_w = off;
         if (op != SPARC_GPU_OP_HAMILTONIAN_APPLY) off += round_up_i64(L->ldw * cb * 8, A);
         L->off_d = off;
-        off += round_up_i64(2 * (int64_t)std::max(c->n_proj_total, 1) * nlb_c_cols(cb) * 8, A);
+        off += round_up_i64(2 * std::max<int64_t>((int64_t)std::max(c->n_proj_total, 1) * nlb_c_cols(cb), nlb_c_doubles(c, cb)) * 8, A);
         L->off_g = off;
         if (op == SPARC_GPU_OP_PROJECT) {
             off += round_up_i64(std::max(gemm_tn_ws_bytes(c, ns, cb, c->nd), gemm_tn_ws_bytes(c, ns, ns, c->nd)), A);
@@ -502,6 +502,8 @@ int sparc_gpu_get_info(const sparc_gpu_ctx *ctx, const char *key, int64_t *value
     if (!strcmp(key, "nl_brick")) { *value = ctx->nlb.ok; return 0; }
     if (!strcmp(key, "nl_brick_blocks")) { *value = ctx->nlb.n_blocks; return 0; }
     if (!strcmp(key, "nl_brick_active")) { *value = ctx->nlb.n_active; return 0; }
+    if (!strcmp(key, "nl_brick_max_blocks")) { *value = ctx->nlb.max_blocks; return 0; }
+    if (!strcmp(key, "nl_brick_max_jobs")) { *value = ctx->nlb.max_jobs; return 0; }
     if (!strncmp(key, "prof_ns:", 8) || !strncmp(key, "prof_count:", 11)) {
         if (!ctx->prof) return SPARC_GPU_OUT_OF_MEMORY;
         const bool is_ns = key[5] == 'n';
@@ -574,11 +576,11 @@ int sparc_gpu_chebyshev_filter(sparc_gpu_ctx *ctx, double *Psi, int64_t ld, int6
         // one degree step: oth <- alpha (H cur - c cur) + beta oth.  With the brick kernel the nonlocal term of step k
         // and the projection chi^T Psi_k needed by step k + 1 share one read-modify-write of oth.
         const int mode = effective_nl_mode(ctx, cur, ldc, oth, ldo);
-        const size_t cbytes = (size_t)ctx->n_proj_total * nlb_c_cols(nb) * 8;
-        double *Cb[2] = {D, D + (int64_t)ctx->n_proj_total * nlb_c_cols(nb)};
-        if (mode == 3) {
+        const size_t cbytes = (size_t)nlb_c_doubles(ctx, nb) * 8;
+        double *Cb[2] = {D, D + nlb_c_doubles(ctx, nb)};
+        if (mode == 3) {     // D_0 = alpha_1 Gamma chi^T Psi_0: the projection folds in the alpha of the step that pulls it
             SPARC_CUDA_TRY(cudaMemsetAsync(Cb[0], 0, cbytes, st));
-            SPARC_TRY(launch_nl_brick(ctx, 1, cur, ldc, nb, 0.0, nullptr, Cb[0], st));
+            SPARC_TRY(launch_nl_brick(ctx, 1, cur, ldc, nb, sigma1 / e, nullptr, Cb[0], st));
         }
         double sigma = sigma1;
         for (int k = 1; k <= degree; ++k) {
@@ -589,7 +591,9 @@ int sparc_gpu_chebyshev_filter(sparc_gpu_ctx *ctx, double *Psi, int64_t ld, int6
             if (mode == 3) {
                 const bool last = (k == degree);
                 if (!last) SPARC_CUDA_TRY(cudaMemsetAsync(Cb[k & 1], 0, cbytes, st));
-                SPARC_TRY(launch_nl_brick(ctx, last ? 2 : 3, oth, ldo, nb, alpha, Cb[(k - 1) & 1], Cb[k & 1], st));
+                // alpha_{k+1} = 2 sigma_{k+1} / e, sigma_{k+1} = 1 / (tau - sigma_k), sigma_k = sigma1 (k = 1) or sigma2
+                const double alpha_next = 2.0 / (tau - (k == 1 ? sigma1 : sigma2)) / e;
+                SPARC_TRY(launch_nl_brick(ctx, last ? 2 : 3, oth, ldo, nb, alpha_next, Cb[(k - 1) & 1], Cb[k & 1], st));
             } else if (mode > 0) {
                 SPARC_TRY(nl_pass_per_atom(ctx, mode, cur, ldc, oth, ldo, nb, alpha, D, st));
             }

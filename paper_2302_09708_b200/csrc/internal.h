@@ -201,12 +201,16 @@ int launch_nl_pull(sparc_gpu_ctx *ctx, const double *D, double *Out, int64_t ldo
 int launch_nl_fused(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double *Out, int64_t ldo, int64_t ncols,
                     double scale, cudaStream_t st);
 
-// Brick-tiled nonlocal kernel (nonlocal_brick.cu).  C buffers hold the raw sums chi_J^T Psi atom-major, element
-// (J, q, col) at po_J * nlb_c_cols(ncols) + col * P_J + q: n_proj_total * nlb_c_cols(ncols) doubles each.
+// Brick-tiled nonlocal kernel (nonlocal_brick.cu).  A C buffer holds D = scale Gamma chi^T Psi as one slab of up to 144 doubles
+// per (atom, 16-column group), in the order of the pull kernel's operand fragments: nlb_c_doubles(ctx, ncols) doubles.
 static inline int64_t nlb_c_cols(int64_t ncols) { return (ncols + 63) / 64 * 64; }
-//   mode 1 (project): c_out += chi^T X                  (X read only; c_out zeroed by the caller)
-//   mode 2 (pull)   : Out += chi (scale Gamma c_in)
-//   mode 3 (both)   : Out += chi (scale Gamma c_in), then c_out += chi^T Out
+static inline int64_t nlb_c_doubles(const sparc_gpu_ctx *c, int64_t ncols)
+{
+    return (int64_t)(c->n_atoms > 0 ? c->n_atoms : 1) * 9 * nlb_c_cols(ncols);
+}
+//   mode 1 (project): c_out += scale Gamma chi^T X        (X read only; c_out zeroed by the caller)
+//   mode 2 (pull)   : Out += chi c_in
+//   mode 3 (both)   : Out += chi c_in, then c_out += scale Gamma chi^T Out   (scale: the alpha of the step that pulls c_out)
 int nlb_build(sparc_gpu_ctx *ctx, const sparc_gpu_desc *d);
 void nlb_free(sparc_gpu_ctx *ctx);
 bool nlb_supported(const sparc_gpu_ctx *ctx, const double *X, int64_t ld);

@@ -64,10 +64,13 @@ struct BrickParams {
     const double *blk;             // [n_blocks][BLK] chi sqrt|gamma| in the shared fragment layout
     double *tile;                  // X (project only) or Out: N_d x ncols, ld
     int64_t ld;
-    // C buffers hold the raw sums (chi sqrt|gamma|)_J^T Psi atom-major: element (J, q, col) at po_J * ncp + col * P_J + q
+    // C buffers hold D = scale sign(gamma) (chi sqrt|gamma|)_J^T Psi, one slab of SLAB doubles per (atom, 16-column group) at
+    // (atom * ngroups16 + group) * SLAB, in the order of the pull's A fragments (CLayout below): the pull reads its operands
+    // with two vector loads and no arithmetic
     const double *c_in;            // of the previous pass (pull)
     double *c_out;                 // accumulated by this pass (project), zeroed by the caller
     int64_t ncp;                   // padded column count of the C buffers (multiple of 64)
+    int32_t ngroups16;             // ncp / 16
     int32_t ncols;
     int32_t ncolgroups;
     int32_t nx, ny, nz;
@@ -75,7 +78,7 @@ struct BrickParams {
     int32_t lhx, lhy;              // log2 of the cube counts along x and y (bx / 2, by / 2)
     int32_t cap_blocks;            // chi blocks the CTA's shared memory holds
     int32_t toct[NB_OCT];          // persistent kernel: byte offset of cube o inside a staged half tile (lane part excluded)
-    double scale;
+    double scale;                  // factor folded into c_out by the projection (the alpha of the degree step that will pull it)
     int32_t dbg;                   // timing experiments only (option "nlb_dbg"): 1 no atomics, 2 no pull math, 4 no project math
 };
 
@@ -95,6 +98,20 @@ template <bool P9> struct BlkLayout {
         if (q == 8) return 64 + pt;
         const int rowpos = ((pt >> 1) & 1) | ((pt & 1) << 1) | (pt & 4);
         return rowpos * 8 + (q ^ (4 * (pt & 1)));
+    }
+};
+
+// Slab of the C buffers: the sums of one atom for one 16-column group, in pull-fragment order.  Slice s = columns 8 s .. 8 s + 7.
+//   P <= 9 class (SLAB = 144): (q < 8, column c, slice s) at 64 s + 2 (4 c + (q & 3)) + (q >> 2): lane (lr = c, lq) of the pull
+//     reads its two k-step operands (q = lq, 4 + lq) as one 16-byte vector; (q = 8, c, s) at 128 + 8 s + c.
+//   P <= 4 class (SLAB = 64): (q, c, s) at 32 s + 4 c + q.
+template <bool P9> struct CLayout {
+    static constexpr int SLAB = P9 ? 144 : 64;
+    __host__ __device__ static int at(int q, int c, int s)
+    {
+        if (!P9) return 32 * s + 4 * c + q;
+        if (q == 8) return 128 + 8 * s + c;
+        return 64 * s + 2 * (4 * c + (q & 3)) + (q >> 2);
     }
 };
 
@@ -138,21 +155,22 @@ __device__ __forceinline__ void run_jobs(double2 (&c)[2][NB_HOCT], const WarpCtx
     constexpr uint32_t BLKB = BlkLayout<P9>::BLK * 8;
     constexpr int KP = P9 ? 2 : 1;
     const int lq = w.lq, lr = w.lr;
-    // A operands of the pull, fetched one job ahead: D_J^T[col, q] = +- scale C_J[q, col]
+    // A operands of the pull, fetched one job ahead: D_J^T[col, q], stored ready-made (scaled, signed, fragment order)
     double nA[2][KP], n8[2];
+    const int64_t gslab = (int64_t)(w.colw >> 4) * CLayout<P9>::SLAB;
     auto fetch_a = [&](int j) {
         const int4 info = jobinfo[j - jbase];
-        const int PJ = info.z;
-        const double *cs = p.c_in + (int64_t)info.w * p.ncp + (w.colw + lr) * PJ;
+        const double *cs = p.c_in + (int64_t)info.w * p.ngroups16 * CLayout<P9>::SLAB + gslab;
 #pragma unroll
         for (int s = 0; s < 2; ++s) {
-            const bool cv = s ? w.cv1 : w.cv0;
-#pragma unroll
-            for (int ks = 0; ks < KP; ++ks) {
-                const int q = 4 * ks + lq;
-                nA[s][ks] = (cv && q < PJ && q < 8) ? cs[s * 8 * PJ + q] : 0.0;
+            if (P9) {
+                const double2 v = *reinterpret_cast<const double2 *>(cs + 64 * s + 2 * (4 * lr + lq));
+                nA[s][0] = v.x; nA[s][KP - 1] = v.y;
+                n8[s] = cs[128 + 8 * s + lr];
+            } else {
+                nA[s][0] = cs[32 * s + 4 * lr + lq];
+                n8[s] = 0.0;
             }
-            n8[s] = (P9 && cv && 8 < PJ) ? cs[s * 8 * PJ + 8] : 0.0;
         }
     };
     if (PULL && r0 < r1) fetch_a(r0);
@@ -169,16 +187,9 @@ __device__ __forceinline__ void run_jobs(double2 (&c)[2][NB_HOCT], const WarpCtx
 
         if (PULL) {
             double dA[2][KP], d8[2];
-            const uint32_t sg = (uint32_t)info.y >> 16;
 #pragma unroll
-            for (int ks = 0; ks < KP; ++ks) {
-                const double sc = ((sg >> (4 * ks + lq)) & 1u) ? -p.scale : p.scale;
-                dA[0][ks] = sc * nA[0][ks]; dA[1][ks] = sc * nA[1][ks];
-            }
-            {
-                const double sc = ((sg >> 8) & 1u) ? -p.scale : p.scale;
-                d8[0] = sc * n8[0]; d8[1] = sc * n8[1];
-            }
+            for (int ks = 0; ks < KP; ++ks) { dA[0][ks] = nA[0][ks]; dA[1][ks] = nA[1][ks]; }
+            d8[0] = n8[0]; d8[1] = n8[1];
             if (j + 1 < r1) fetch_a(j + 1);
             if (mask && !(p.dbg & 2)) {
                 // operands of the next block are fetched while the current block's DMMAs issue (reading one block
@@ -197,17 +208,19 @@ __device__ __forceinline__ void run_jobs(double2 (&c)[2][NB_HOCT], const WarpCtx
                         nb0 = lds1(aA);
                         if (KP > 1) nb1 = lds1(aA ^ 32u);
                         if (P9) nx8 = lds2(aX);
-                        dmma884(c[0][o].x, c[0][o].y, dA[0][0], b0);
-                        dmma884(c[1][o].x, c[1][o].y, dA[1][0], b0);
-                        if (KP > 1) {
-                            dmma884(c[0][o].x, c[0][o].y, dA[0][KP - 1], b1);
-                            dmma884(c[1][o].x, c[1][o].y, dA[1][KP - 1], b1);
-                        }
+                        // the rank-1 update of projector 8 goes FIRST: a DFMA behind the DMMAs of the same accumulator would
+                        // wait out their 26-cycle latency with the (in-order) warp unable to issue the next octet
                         if (P9) {
                             c[0][o].x = fma(d8[0], x8.x, c[0][o].x);
                             c[0][o].y = fma(d8[0], x8.y, c[0][o].y);
                             c[1][o].x = fma(d8[1], x8.x, c[1][o].x);
                             c[1][o].y = fma(d8[1], x8.y, c[1][o].y);
+                        }
+                        dmma884(c[0][o].x, c[0][o].y, dA[0][0], b0);
+                        dmma884(c[1][o].x, c[1][o].y, dA[1][0], b0);
+                        if (KP > 1) {
+                            dmma884(c[0][o].x, c[0][o].y, dA[0][KP - 1], b1);
+                            dmma884(c[1][o].x, c[1][o].y, dA[1][KP - 1], b1);
                         }
                     }
                 }
@@ -243,48 +256,47 @@ __device__ __forceinline__ void run_jobs(double2 (&c)[2][NB_HOCT], const WarpCtx
                     }
                 }
             }
+            // the lane holds rows q = lr of C_J for columns 2 lq, 2 lq + 1 of each slice; they leave as D = +- scale C in the slab
+            // order of CLayout (rows q >= P_J are exact zeros: the blocks carry zeros there)
+            const uint32_t sg = (uint32_t)info.y >> 16;
+            const double sc = ((sg >> lr) & 1u) ? -p.scale : p.scale;
+            const double sc8 = ((sg >> 8) & 1u) ? -p.scale : p.scale;
+            const int64_t slab_g = ((int64_t)info.w * p.ngroups16 + (w.colw >> 4)) * CLayout<P9>::SLAB;
+            double v8[2] = {0.0, 0.0};
+            if (P9) {
+#pragma unroll
+                for (int s = 0; s < 2; ++s) {
+                    double v = p8[s][0] + p8[s][1];
+                    v += __shfl_xor_sync(0xffffffffu, v, 1);
+                    v += __shfl_xor_sync(0xffffffffu, v, 2);
+                    v8[s] = sc8 * v;                                              // lanes lq == 0 .. 3 all hold column lr
+                }
+            }
             if (stage) {
-                // the slab [col][q] (16 x P_J doubles, contiguous in C) is staged in shared memory and reduced in one copy
+                // staged in shared memory and added to the atom's slab with one bulk reduction (UBLKRED.ADD.F64)
                 if (w.lq == 0 && w.lr == 0) tma_store_wait_read_all();           // the previous job's copy has read the slab
                 __syncwarp();
 #pragma unroll
                 for (int s = 0; s < 2; ++s) {
-                    const uint32_t a = stage + (uint32_t)(((8 * s + 2 * lq) * PJ + lr) * 8);
-                    if (lr < PJ && lr < 8) {
-                        sts1(a, acc[s][0][0] + acc[s][1][0]);
-                        sts1(a + (uint32_t)PJ * 8u, acc[s][0][1] + acc[s][1][1]);
+                    if (w.bval) {
+                        sts1(stage + (uint32_t)(CLayout<P9>::at(lr, 2 * lq, s) * 8), sc * (acc[s][0][0] + acc[s][1][0]));
+                        sts1(stage + (uint32_t)(CLayout<P9>::at(lr, 2 * lq + 1, s) * 8), sc * (acc[s][0][1] + acc[s][1][1]));
                     }
-                    if (P9) {
-                        double v = p8[s][0] + p8[s][1];
-                        v += __shfl_xor_sync(0xffffffffu, v, 1);
-                        v += __shfl_xor_sync(0xffffffffu, v, 2);
-                        if (lq == 0 && 8 < PJ) sts1(stage + (uint32_t)(((8 * s + lr) * PJ + 8) * 8), v);
-                    }
+                    if (P9 && lq == 0) sts1(stage + (uint32_t)(CLayout<P9>::at(8, lr, s) * 8), v8[s]);
                 }
                 fence_async_smem();
                 __syncwarp();
                 if (w.lq == 0 && w.lr == 0 && !(p.dbg & 1))
-                    bulk_reduce_add_f64(p.c_out + (int64_t)info.w * p.ncp + (int64_t)w.colw * PJ, stage, (uint32_t)(16 * PJ * 8));
+                    bulk_reduce_add_f64(p.c_out + slab_g, stage, (uint32_t)(CLayout<P9>::SLAB * 8));
             } else if (!(p.dbg & 1)) {
-                // element (q, col) of the atom's slab at col * P_J + q
-                double *cout = p.c_out + (int64_t)info.w * p.ncp + (w.colw + 2 * lq) * PJ + lr;
+                double *cout = p.c_out + slab_g;
 #pragma unroll
                 for (int s = 0; s < 2; ++s) {
-                    const double v0 = acc[s][0][0] + acc[s][1][0];
-                    const double v1 = acc[s][0][1] + acc[s][1][1];
-                    const int ca = w.colw + 8 * s + 2 * lq;
-                    if (lr < PJ && lr < 8) {
-                        if (ca < p.ncols) atomicAdd(cout + 8 * s * PJ, v0);
-                        if (ca + 1 < p.ncols) atomicAdd(cout + (8 * s + 1) * PJ, v1);
+                    if (w.bval) {
+                        atomicAdd(cout + CLayout<P9>::at(lr, 2 * lq, s), sc * (acc[s][0][0] + acc[s][1][0]));
+                        atomicAdd(cout + CLayout<P9>::at(lr, 2 * lq + 1, s), sc * (acc[s][0][1] + acc[s][1][1]));
                     }
-                    if (P9) {
-                        double v = p8[s][0] + p8[s][1];
-                        v += __shfl_xor_sync(0xffffffffu, v, 1);
-                        v += __shfl_xor_sync(0xffffffffu, v, 2);
-                        const int col = w.colw + 8 * s + lr;
-                        if (lq == 0 && col < p.ncols && 8 < PJ)
-                            atomicAdd(p.c_out + (int64_t)info.w * p.ncp + col * PJ + 8, v);
-                    }
+                    if (P9 && lq == 0) atomicAdd(cout + CLayout<P9>::at(8, lr, s), v8[s]);
                 }
             }
         }
@@ -311,7 +323,7 @@ __device__ __forceinline__ void load_round(const BrickParams &p, int j0, int na,
     const bool take = jm < na && incl <= p.cap_blocks;
     const int cnt = __popc(__ballot_sync(0xffffffffu, take));      // a prefix: incl is non-decreasing
     if (take) {
-        jobinfo[lane] = make_int4(incl - nb, (int)job.mask, job.pj, job.po);
+        jobinfo[lane] = make_int4(incl - nb, (int)job.mask, job.pj, job.atom);
         if (p.dbg & 16) mbar_arrive(&full[lane]);
         else {
             mbar_arrive_expect_tx(&full[lane], (uint32_t)(nb * BLK * 8));
@@ -416,7 +428,7 @@ constexpr int NLP_WARPS = 16;
 constexpr int NLP_COLS = 16;                                  // columns per item
 constexpr int NLP_GSTEP = NLP_WARPS / 2;                      // column groups in flight per half
 constexpr int NLP_TILE_BYTES = (NB_PTS / 2) * NLP_COLS * 8;   // 8 KB
-constexpr int NLP_SLAB_BYTES = NLP_COLS * 9 * 8;              // 16 columns x P_J <= 9 partial sums of one job
+constexpr int NLP_SLAB_BYTES = CLayout<true>::SLAB * 8;         // one slab: 16 columns x 9 sums of one job
 
 template <bool P9, bool DO_PULL, bool DO_PROJ>
 __global__ void __launch_bounds__(NLP_WARPS * 32, 1)
@@ -772,6 +784,7 @@ int launch_nl_brick(sparc_gpu_ctx *ctx, int mode, double *XorOut, int64_t ld, in
     P.tile = XorOut; P.ld = ld;
     P.c_in = c_in; P.c_out = c_out;
     P.ncp = nlb_c_cols(ncols);
+    P.ngroups16 = (int32_t)(P.ncp / 16);
     P.ncols = (int32_t)ncols;
     P.nx = ctx->n[0]; P.ny = ctx->n[1]; P.nz = ctx->n[2];
     P.bx = B.bx; P.by = B.by;
