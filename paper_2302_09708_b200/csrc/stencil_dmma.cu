@@ -45,6 +45,11 @@ struct DmParams {
     int ytiles, zchunks, zchunk_len;
     int per_x, per_y, per_z;
     uint32_t psi_bytes, tile_bytes, stage_bytes;
+    // x tiling (grids wider than 96 points): nxt tiles of xt columns (a multiple of 8; the last may overhang); every tile then
+    // stores 6 halo columns on either side (x_start = tile start - 6); on a periodic x axis the first / last tile gets the
+    // wrapped columns as two extra 8-column boxes behind the Veff / Prev tiles
+    int nxt, xt;
+    uint32_t halo_bytes;      // one 8-column x TY-row halo box
 };
 
 using namespace sm100;
@@ -54,7 +59,7 @@ template <bool HAS_PREV, int TYB, int MINB>
 __global__ void __launch_bounds__(MINB == 1 ? 13 * 32 : 7 * 32, MINB)
 stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
                     const __grid_constant__ CUtensorMap tmap_v, const __grid_constant__ CUtensorMap tmap_p,
-                    const __grid_constant__ DmParams P)
+                    const __grid_constant__ CUtensorMap tmap_h, const __grid_constant__ DmParams P)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t *bar_full = reinterpret_cast<uint64_t *>(smem_raw);    // [MAX_STAGES] TMA landed
@@ -72,11 +77,17 @@ stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
     }
     __syncthreads();
 
-    const int per_col = P.ytiles * P.zchunks;
+    const int per_col = P.ytiles * P.zchunks * P.nxt;
     const int col = blockIdx.x / per_col;
-    const int rem = blockIdx.x - col * per_col;
+    int rem = blockIdx.x - col * per_col;
+    const int xtile = rem % P.nxt;               // x tiles of one (column, y tile, z chunk) are neighbours in the grid
+    rem /= P.nxt;
     const int ytile = rem / P.zchunks;
     const int zc = rem - ytile * P.zchunks;
+    const bool tiled = P.nxt > 1;
+    const int xt0 = xtile * P.xt;
+    const bool halo_l = tiled && P.per_x && xtile == 0, halo_r = tiled && P.per_x && xtile == P.nxt - 1;
+    const uint32_t halo_off = P.psi_bytes + 2 * P.tile_bytes;     // left box, then right box
     const int y0 = ytile * TY;
     const int z0 = zc * P.zchunk_len;
     const int z1 = min(z0 + P.zchunk_len, P.nz);
@@ -90,6 +101,7 @@ stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
         prefetch_tmap(&tmap_x8);
         prefetch_tmap(&tmap_v);
         if (HAS_PREV) prefetch_tmap(&tmap_p);
+        const int xs = tiled ? xt0 - R : P.x_start, xv = tiled ? xt0 : 0;
         const uint32_t row_bytes = (uint32_t)(W * 8);
         const uint32_t tile_tx = (uint32_t)(TY * W * 8);
         // TYB + 2 boxes of 8 rows (128-byte aligned destinations): rows y0-8 .. y0-1 (6 used), the tile, y0+TY ..
@@ -108,14 +120,18 @@ stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
             int zin = z0 - R + s;
             if (P.per_z) { if (zin < 0) zin += P.nz; else if (zin >= P.nz) zin -= P.nz; }
             const uint32_t dst = stage0 + (uint32_t)stage * P.stage_bytes;
-            mbar_arrive_expect_tx(&bar_full[stage], P.psi_bytes + (do_xy ? tile_tx : 0u) + (do_prev ? tile_tx : 0u));
-            tma_load_4d(dst, &tmap_x8, &bar_full[stage], P.x_start, yt, zin, col);
+            mbar_arrive_expect_tx(&bar_full[stage], P.psi_bytes + (do_xy ? tile_tx : 0u) + (do_prev ? tile_tx : 0u) +
+                                                        ((do_xy && halo_l) ? P.halo_bytes : 0u) + ((do_xy && halo_r) ? P.halo_bytes : 0u));
+            tma_load_4d(dst, &tmap_x8, &bar_full[stage], xs, yt, zin, col);
 #pragma unroll
             for (int j = 0; j < TYB; ++j)
-                tma_load_4d(dst + (1 + j) * TB * row_bytes, &tmap_x8, &bar_full[stage], P.x_start, y0 + TB * j, zin, col);
-            tma_load_4d(dst + (1 + TYB) * TB * row_bytes, &tmap_x8, &bar_full[stage], P.x_start, yb, zin, col);
-            if (do_xy) tma_load_3d(dst + P.psi_bytes, &tmap_v, &bar_full[stage], 0, y0, z0 - R + s);
-            if (do_prev) tma_load_4d(dst + P.psi_bytes + P.tile_bytes, &tmap_p, &bar_full[stage], 0, y0, z0 - 2 * R + s, col);
+                tma_load_4d(dst + (1 + j) * TB * row_bytes, &tmap_x8, &bar_full[stage], xs, y0 + TB * j, zin, col);
+            tma_load_4d(dst + (1 + TYB) * TB * row_bytes, &tmap_x8, &bar_full[stage], xs, yb, zin, col);
+            if (do_xy) tma_load_3d(dst + P.psi_bytes, &tmap_v, &bar_full[stage], xv, y0, z0 - R + s);
+            if (do_prev) tma_load_4d(dst + P.psi_bytes + P.tile_bytes, &tmap_p, &bar_full[stage], xv, y0, z0 - 2 * R + s, col);
+            // wrapped x halo of the centre plane's tile rows: columns nx-8 .. nx-1 (left), 0 .. 7 (right)
+            if (do_xy && halo_l) tma_load_4d(dst + halo_off, &tmap_h, &bar_full[stage], P.nx - 8, y0, zin, col);
+            if (do_xy && halo_r) tma_load_4d(dst + halo_off + P.halo_bytes, &tmap_h, &bar_full[stage], 0, y0, zin, col);
             if (++stage == P.nstage) { stage = 0; phase ^= 1u; }
         }
         return;
@@ -128,8 +144,8 @@ stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
     const int rb = cw / P.nxb;                  // 8-row block of the tile
     const int x0 = 8 * (cw - rb * P.nxb);
     const int ry = TB * rb;
-    const bool xvalid = x0 + 2 * (lane & 3) < P.nx;       // n_x is even: a lane's pair is inside or outside as a whole
-    const int xoff = P.per_x ? 0 : R;           // halo columns are stored only for a Dirichlet x axis
+    const bool xvalid = xt0 + x0 + 2 * (lane & 3) < P.nx;       // n_x is even: a lane's pair is inside or outside as a whole
+    const int xoff = (P.per_x && !tiled) ? 0 : R;    // halo columns are stored for a Dirichlet x axis and for x tiles
     // Toeplitz fragments: tap distance d = (k - 6) - (output index), k = 4 s + lq; the centre tap is pointwise
     double ay[KS];                              // (the x fragments are rxy times the same numbers)
     uint32_t xa[KS];                            // byte offsets of the x-tap data fragments (row y0 + lr, wrapped column)
@@ -139,16 +155,23 @@ stencil_dmma_kernel(const __grid_constant__ CUtensorMap tmap_x8,
         const int ad = d < 0 ? -d : d;
         ay[s] = (ad >= 1 && ad <= R) ? P.cy[ad] : 0.0;
         int xc = x0 - R + 4 * s + lq;
-        if (P.per_x) { if (xc < 0) xc += P.nx; else if (xc >= P.nx) xc -= P.nx; }
-        else xc += R;
-        xa[s] = (uint32_t)(((TB + ry + lr) * W + xc) * 8);
+        if (!tiled) {
+            if (P.per_x) { if (xc < 0) xc += P.nx; else if (xc >= P.nx) xc -= P.nx; }
+            else xc += R;
+            xa[s] = (uint32_t)(((TB + ry + lr) * W + xc) * 8);
+        } else {
+            const int xg = xt0 + xc;                                        // global column of this fragment element
+            if (halo_l && xg < 0) xa[s] = halo_off + (uint32_t)(((ry + lr) * 8 + xg + 8) * 8);
+            else if (halo_r && xg >= P.nx && xg < P.nx + 8) xa[s] = halo_off + P.halo_bytes + (uint32_t)(((ry + lr) * 8 + xg - P.nx) * 8);
+            else xa[s] = (uint32_t)(((TB + ry + lr) * W + xc + R) * 8);    // inside the box (zero-filled outside a Dirichlet face)
+        }
     }
     const uint32_t ya0 = (uint32_t)(((TB - R + ry + lq) * W + x0 + lr + xoff) * 8);      // row y0 + ry - 6 + lq, + s * 4 rows
     const uint32_t ystep = (uint32_t)(4 * W * 8);
     const uint32_t own_off = (uint32_t)(((TB + ry + lr) * W + x0 + 2 * lq + xoff) * 8);
     const uint32_t tile_off = P.psi_bytes + (uint32_t)(((ry + lr) * W + x0 + 2 * lq) * 8);
     const int64_t plane = (int64_t)P.nx * P.ny;
-    double *out_z = P.out + (int64_t)col * P.ldo + (int64_t)(y0 + ry + lr) * P.nx + x0 + 2 * lq + (int64_t)(z0 - 2 * R) * plane;
+    double *out_z = P.out + (int64_t)col * P.ldo + (int64_t)(y0 + ry + lr) * P.nx + xt0 + x0 + 2 * lq + (int64_t)(z0 - 2 * R) * plane;
 
     double acc[NSLOT][2];
 #pragma unroll
@@ -243,9 +266,9 @@ bool stencil_dmma_supported(const sparc_gpu_ctx *ctx, const double *X, int64_t l
 {
     if (!ctx->fn_encode_tiled || ctx->radius != R) return false;
     const int nx = ctx->n[0], ny = ctx->n[1];
-    if (nx % 2 || nx < 16 || nx > 96) return false;          // <= 12 consumer warps
+    if (nx % 2 || nx < 16) return false;                     // wider than 96 points: x tiles
     if (ny % TB || ny < 2 * TB) return false;
-    if (pick_pitch((nx + 7) / 8 * 8 + (ctx->bc[0] == 0 ? 0 : 2 * R)) > 256) return false;
+    if (nx <= 96 && pick_pitch((nx + 7) / 8 * 8 + (ctx->bc[0] == 0 ? 0 : 2 * R)) > 256) return false;
     if (!a16(X) || !a16(Out) || (Prev && !a16(Prev)) || (ldx & 1) || (ldo & 1) || (Prev && (ldp & 1))) return false;
     return true;
 }
@@ -264,10 +287,28 @@ int launch_stencil_dmma(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double
     P.ldo = ldo;
     P.nx = nx; P.ny = ny; P.nz = nz;
     P.per_x = ctx->bc[0] == 0; P.per_y = ctx->bc[1] == 0; P.per_z = ctx->bc[2] == 0;
-    P.W = pick_pitch(8 * ((nx + 7) / 8) + (P.per_x ? 0 : 2 * R));
-    P.x_start = P.per_x ? 0 : -R;
+    // x tiling for grids wider than 96 points (12 consumer warps): tile width a multiple of 8.  Measured at n_x = 128 (config 5,
+    // stencil only): 2 x 64 and 4 x 32 reach 3.7 TB/s, 3 x 48 (16 columns of overhang) 3.3, 2 x 96 (64 of overhang) 3.0 -- the
+    // overhang of the last tile costs more than anything else, 8 resident consumer warps are enough, and every tile re-reads
+    // 12 halo columns
+    P.nxt = 1; P.xt = 8 * ((nx + 7) / 8);
+    if (nx > 96) {
+        double best = -1.0;
+        for (int xt = 96; xt >= 32; xt -= 8) {
+            const int nxt = (nx + xt - 1) / xt, warps = xt / 8;
+            const double useful = nx / ((double)nxt * xt);
+            const double score = std::min((warps <= 6 ? 2.0 : 1.0) * warps, 8.0) * useful * useful * useful * xt / (xt + R);
+            if (score > best) { best = score; P.xt = xt; P.nxt = nxt; }
+        }
+        if (ctx->opt_stencil_xt >= 32 && ctx->opt_stencil_xt <= 96 && ctx->opt_stencil_xt % 8 == 0) {
+            P.xt = ctx->opt_stencil_xt; P.nxt = (nx + P.xt - 1) / P.xt;
+        }
+    }
+    const bool tiled = P.nxt > 1;
+    P.W = pick_pitch(P.xt + ((P.per_x && !tiled) ? 0 : 2 * R));
+    P.x_start = (P.per_x && !tiled) ? 0 : -R;
     // 16-row tiles (a third less halo traffic) when 2 nx / 8 consumer warps still fit the 12-warp kernel
-    const int nxb = (nx + 7) / 8;
+    const int nxb = P.xt / 8;
     const int tyb = (ctx->opt_stencil_ty == 16 && ny % (2 * TB) == 0 && 2 * nxb <= 12) ? 2 : 1;
     const int TY = TB * tyb;
     P.nxb = nxb;
@@ -275,13 +316,14 @@ int launch_stencil_dmma(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double
     P.ytiles = ny / TY;
     P.psi_bytes = (uint32_t)((tyb + 2) * TB * P.W * 8);
     P.tile_bytes = (uint32_t)(TY * P.W * 8);
-    P.stage_bytes = P.psi_bytes + 2 * P.tile_bytes;
+    P.halo_bytes = (uint32_t)(8 * TY * 8);
+    P.stage_bytes = P.psi_bytes + 2 * P.tile_bytes + ((tiled && P.per_x) ? 2 * P.halo_bytes : 0u);
     const int threads = (P.nwarps + 1) * 32;
     // one 8-row block and up to 6 consumer warps: two CTAs per SM (128 registers; a third would need <= 80 and spills the
     // z-sums); otherwise one CTA of up to 12 consumer warps.  The kernel's TYB must be the one the parameters (boxes per
     // stage, y tiles, warps) were built for, so it is chosen from tyb first.
     const bool small = tyb == 1 && P.nwarps <= 6;
-    typedef void (*Kern)(const CUtensorMap, const CUtensorMap, const CUtensorMap, const DmParams);
+    typedef void (*Kern)(const CUtensorMap, const CUtensorMap, const CUtensorMap, const CUtensorMap, const DmParams);
     Kern kern = tyb == 2 ? (has_prev ? (Kern)stencil_dmma_kernel<true, 2, 1> : (Kern)stencil_dmma_kernel<false, 2, 1>)
                 : small  ? (has_prev ? (Kern)stencil_dmma_kernel<true, 1, 2> : (Kern)stencil_dmma_kernel<false, 1, 2>)
                          : (has_prev ? (Kern)stencil_dmma_kernel<true, 1, 1> : (Kern)stencil_dmma_kernel<false, 1, 1>);
@@ -298,24 +340,25 @@ int launch_stencil_dmma(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double
 
     CUtensorMap tmap_v;
     if (!encode_map(ctx, &tmap_v, ctx->d_veff, 3, 1, ctx->nd, P.W, TY)) return SPARC_GPU_CUDA_ERROR;   // whole tile
-    const int64_t max_cols_per_launch = std::max<int64_t>(1, (int64_t)INT32_MAX / ((int64_t)P.ytiles * nz));
+    const int64_t max_cols_per_launch = std::max<int64_t>(1, (int64_t)INT32_MAX / ((int64_t)P.ytiles * nz * P.nxt));
     for (int64_t j0 = 0; j0 < ncols; j0 += max_cols_per_launch) {
         const int64_t nb = std::min<int64_t>(max_cols_per_launch, ncols - j0);
         int zchunks = 1;
-        const int64_t base = nb * P.ytiles;
+        const int64_t base = nb * P.ytiles * P.nxt;
         const int64_t want = 2LL * ctx->sm_count * ctas;
         if (base < want) zchunks = (int)std::min<int64_t>((want + base - 1) / base, std::max(1, nz / 12));
         if (ctx->opt_stencil_zchunks > 0) zchunks = std::min(ctx->opt_stencil_zchunks, nz);
         P.zchunk_len = (nz + zchunks - 1) / zchunks;
         P.zchunks = (nz + P.zchunk_len - 1) / P.zchunk_len;
         P.out = Out + j0 * ldo;
-        CUtensorMap tmap_x, tmap_p;
+        CUtensorMap tmap_x, tmap_p, tmap_h;
         if (!encode_map(ctx, &tmap_x, X + j0 * ldx, 4, nb, ldx, P.W, TB)) return SPARC_GPU_CUDA_ERROR;
+        if (!encode_map(ctx, &tmap_h, X + j0 * ldx, 4, nb, ldx, 8, TY)) return SPARC_GPU_CUDA_ERROR;
         if (!encode_map(ctx, &tmap_p, has_prev ? Prev + j0 * ldp : X + j0 * ldx, 4, nb, has_prev ? ldp : ldx, P.W, TY))
             return SPARC_GPU_CUDA_ERROR;
-        const unsigned grid = (unsigned)(nb * P.ytiles * P.zchunks);
+        const unsigned grid = (unsigned)(nb * P.ytiles * P.zchunks * P.nxt);
         prof_begin(ctx, KK_STENCIL_TMA, st);
-        kern<<<grid, threads, smem, st>>>(tmap_x, tmap_v, tmap_p, P);
+        kern<<<grid, threads, smem, st>>>(tmap_x, tmap_v, tmap_p, tmap_h, P);
         prof_end(ctx, KK_STENCIL_TMA, st);
     }
     SPARC_CUDA_TRY(cudaGetLastError());

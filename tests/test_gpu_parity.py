@@ -100,7 +100,10 @@ def test_h_apply_and_filter_small(torch, api, wl, path):
 
 
 @pytest.mark.parametrize("bc", [(0, 0, 0), (1, 1, 1), (0, 1, 0), (1, 0, 1), (0, 0, 1)])
-@pytest.mark.parametrize("n", [(24, 16, 17), (16, 24, 30), (40, 32, 14), (72, 16, 13), (96, 24, 14), (60, 16, 13), (26, 16, 14)])
+@pytest.mark.parametrize("n", [(24, 16, 17), (16, 24, 30), (40, 32, 14), (72, 16, 13), (96, 24, 14), (60, 16, 13), (26, 16, 14),
+                               # wider than 96 points: x tiles (3 x 48 with an overhanging last tile; 2 x 56 -> 3 tiles; 3 x 48
+                               # exact; ragged 106)
+                               (128, 16, 13), (112, 16, 14), (144, 16, 13), (106, 24, 13)])
 def test_stencil_dmma_path(torch, api, n, bc):
     """Hybrid stencil kernel (in-plane taps as DMMA Toeplitz products, stencil_path = 3) against the oracle: periodic
     wraps and Dirichlet faces on every axis, anisotropic spacing, several x blocks and y tiles, ragged z."""
