@@ -40,10 +40,12 @@ METRIC = "CheFSI filter grid-pt·orbital·degree/s + HBM GB/s; subspace FP64 TFL
 UNIT = "grid-pt*orbital*degree/s"
 ALG_BYTES_PER_UNIT = 24.0       # read Psi_k, read Psi_{k-1}, write Psi_{k+1}
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` captures, keyed by (config, kernel).
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {(1, "stencil"): 697.6e6,       # profiles/r01b_ncu_kernels_cfg1.md
-                                (3, "stencil"): 23.32e9}       # profiles/r01c_ncu_kernels_cfg3.md (hybrid kernel)
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the kernel, from the committed `ncu --set full` captures
+# (profiles/r02_ncu_kernels.md), keyed by (config, kernel).  The GEMM entry is the capture of the seventh column block of
+# Hs at config 4 (556 ms; the launches differ: tiles below the diagonal are skipped).
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {(4, "gemm_tn"): 1.0438e12, (4, "nonlocal"): 31.415e9, (4, "stencil"): 34.596e9,
+                                (1, "stencil"): 696.99e6, (1, "nonlocal"): 260.2e6, (2, "stencil"): 16.145e9,
+                                (5, "stencil"): 57.59e9}
 
 
 def measured_peaks():

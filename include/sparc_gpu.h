@@ -12,11 +12,14 @@
  *   components" of the orbitals.  On top of H:
  *     - the Chebyshev filter  X <- p_m((H - cI)/e) X
  *     - the projection        Hs = X^T H X,  Ms = X^T X
- *     - the rotation          X <- X Q   (Q = eigenvectors supplied by the caller; the N_s x N_s
- *                             eigensolve, is outside this library)
+ *     - the rotation          X <- X Q   (Q = eigenvectors supplied by the caller, or computed on the device by
+ *                             sparc_gpu_eigensolve)
+ *   and: the gradient stencil / projector contraction / nonlocal force, the subspace
+ *   eigensolve, the complex k-point variants (*_k) and the local pieces of the multi-GPU row partition.
  *
  * Conventions
- *   - Real FP64 only (Gamma point).  Grid linear index i = x + nx*(y + ny*z).
+ *   - FP64 throughout; real orbitals (Gamma point) except in the *_k entry points (complex, interleaved
+ *     re/im).  Grid linear index i = x + nx*(y + ny*z).
  *   - Psi, X, Y: N_d x ncols, column-major, leading dimension ld >= N_d; one column = one orbital.
  *     Hs, Ms, Q: ns x ns, column-major, ld = ns.
  *   - Pointers named *_dev are DEVICE pointers owned by the caller (e.g. PyTorch tensors); pointers in
@@ -256,12 +259,14 @@ int sparc_gpu_probe_peak(int device, int kind, double *value_out, void *scratch_
  *   "nonlocal"        1 on, 0 off: drops V_nl (used by closed-form pins)
  *   "nonlocal_mode"   0 auto (brick-tiled DMMA kernel when supported, else 2), 1 project + pull: bitwise reproducible,
  *                     2 per-atom kernel with atomic scatter, 3 brick kernel or UNSUPPORTED
- *   "nlb_variant"     brick kernel shape: 0 = 32 columns per CTA, three CTAs per SM; 1 = 32 columns, four CTAs;
- *                     2 = 64 columns, two CTAs
+ *   "nlb_kernel"      brick kernel: 0 auto (persistent kernel when every brick's chi blocks fit its store), 1 general
+ *                     kernel, 2 persistent kernel or UNSUPPORTED;  "nlb_cap" (test knob): cap on the chi blocks kept in
+ *                     shared memory by the general kernel (forces load rounds);  "nlb_dbg": timing experiments only
  *   "gemm_path"       0 auto, 1 simple FMA kernel, 2 DMMA kernel
  *   "gemm_full"       0: Hs, Ms as upper-triangle tiles + mirror (R12), 1: all tiles
  *   "stencil_ay" (0 auto, 1, 2), "stencil_ty" (0 auto, else tile rows), "stencil_stages" (0 auto, 2..8 TMA ring depth),
- *   "stencil_zchunks" (0 auto): tile knobs of the stencil kernels
+ *   "stencil_zchunks" (0 auto), "stencil_xt" (0 auto, else 32..96 multiple of 8: x-tile width of the hybrid kernel on grids
+ *   wider than 96 points): tile knobs of the stencil kernels
  *   "profile" (0 / 1), "profile_reset": per-kernel CUDA-event timing, read back through sparc_gpu_get_info */
 int sparc_gpu_set_option(sparc_gpu_ctx *ctx, const char *key, int64_t value);
 
@@ -269,10 +274,11 @@ int sparc_gpu_set_option(sparc_gpu_ctx *ctx, const char *key, int64_t value);
  *   "kernel_launches" (cumulative kernels launched by this context), "nd", "n_proj_total", "covered_points", "sm_count",
  *   "stencil_path_last" (1 generic, 2 TMA + DFMA, 3 TMA + DMMA hybrid: the kernel the last local pass used),
  *   "nl_brick" (1: the brick tables exist), "nl_brick_blocks", "nl_brick_active" (chi blocks / bricks with work),
+ *   "nl_brick_max_blocks", "nl_brick_max_jobs" (most chi blocks / atoms of any one brick),
  *   "gemm_tn_mflop", "gemm_nn_mflop" (flop issued by the DMMA GEMMs since the last "profile_reset", in 1e6),
  *   "prof_count:<k>" launches and "prof_ns:<k>" summed nanoseconds of kernel kind k since the last "profile_reset"
  *   (k: 0 generic stencil, 1 TMA stencils, 2 nl project, 3 nl pull, 4 GEMM TN, 5 GEMM NN, 6 split-K reduce, 7 copies /
- *   mirror, 8 per-atom nonlocal, 9 brick nonlocal, 10 gradient stencil, 11 eigensolver kernels).  "prof_ns:<k>" waits for
+ *   mirror, 8 per-atom nonlocal, 9 brick nonlocal, 10 gradient stencil / force contraction, 11 eigensolver kernels, 12 k-point kernels).  "prof_ns:<k>" waits for
  *   the recorded events (cudaEventSynchronize): the one get_info key that blocks. */
 int sparc_gpu_get_info(const sparc_gpu_ctx *ctx, const char *key, int64_t *value);
 

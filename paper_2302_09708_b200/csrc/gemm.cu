@@ -160,11 +160,15 @@ gemm_dmma_kernel(const double *__restrict__ A, int64_t lda, const double *__rest
     }
 }
 
+// diag >= 0: the GEMM skipped the 128 x BN tiles strictly below the diagonal of a symmetric result (m0 >= diag + n0 + BN);
+// their partials were never written and are not read here (launch_mirror_upper fills those elements of C afterwards)
 __global__ void __launch_bounds__(256)
-splitk_reduce_kernel(const double *__restrict__ part, int splits, int64_t M, int64_t N, double *C, int64_t ldc)
+splitk_reduce_kernel(const double *__restrict__ part, int splits, int64_t M, int64_t N, double *C, int64_t ldc, int64_t diag,
+                     int bn)
 {
     const int64_t total = M * N;
     for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x) {
+        if (diag >= 0 && ((e % M) / BM) * BM >= diag + ((e / M) / bn) * bn + bn) continue;
         double s = 0.0;
         for (int z = 0; z < splits; ++z) s += part[(int64_t)z * total + e];     // fixed order: deterministic
         C[(e % M) + (e / M) * ldc] = s;
@@ -303,7 +307,7 @@ int launch_gemm_tn(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const doubl
         SPARC_TRY(launch_dmma<false>(ctx, A, lda, B, ldb, part, M, M, N, K, plan, diag, st));     // skipped tiles stay undefined
         int64_t blocks = std::min<int64_t>((M * N + 255) / 256, (int64_t)ctx->sm_count * 8);
         prof_begin(ctx, KK_SPLITK_REDUCE, st);
-        splitk_reduce_kernel<<<(unsigned)blocks, 256, 0, st>>>(part, plan.splits, M, N, C, ldc);
+        splitk_reduce_kernel<<<(unsigned)blocks, 256, 0, st>>>(part, plan.splits, M, N, C, ldc, diag, 32 * NWN_DEFAULT);
         prof_end(ctx, KK_SPLITK_REDUCE, st);
         SPARC_CUDA_TRY(cudaGetLastError());
         return SPARC_GPU_SUCCESS;

@@ -336,7 +336,12 @@ int launch_stencil_dmma(sparc_gpu_ctx *ctx, const double *X, int64_t ldx, double
     if (nstage < 2) return SPARC_GPU_UNSUPPORTED;
     P.nstage = nstage;
     const size_t smem = 512 + (size_t)nstage * P.stage_bytes;
-    SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    // once per context and kernel variant (the attribute is per device and function; the maximum any launch may ask for)
+    const int vbit = 20 + (tyb == 2 ? 0 : small ? 2 : 4) + (has_prev ? 1 : 0);
+    if (!(ctx->func_attr_done & (1ull << vbit))) {
+        SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        ctx->func_attr_done |= 1ull << vbit;
+    }
 
     CUtensorMap tmap_v;
     if (!encode_map(ctx, &tmap_v, ctx->d_veff, 3, 1, ctx->nd, P.W, TY)) return SPARC_GPU_CUDA_ERROR;   // whole tile
