@@ -10,6 +10,7 @@
 //         sigma = 1.05 max_i sum_j |A_ij| (Gershgorin: A + sigma I is positive definite with condition number <= 41),
 //         A + sigma I = R R^T,  G = R^T  (so G^T G = A + sigma I);  plane rotations G <- G J, V <- V J make the columns of G
 //         mutually orthogonal: then V^T (A + sigma I) V = diag(|g_j|^2), i.e. V = eigenvectors, |g_j|^2 - sigma = eigenvalues.
+//         V is not accumulated during the sweeps: G_final = R^T V, so V = R^-T G_final (one back substitution).
 //       Pairs follow the round-robin (tournament) ordering: n/2 disjoint column pairs per round, n - 1 rounds per sweep, one
 //       CTA per pair.  Only whole columns are touched, so every access is a contiguous run (a two-sided Jacobi would also
 //       rotate rows).  Jacobi on the Cholesky factor converges in few sweeps (Veselic-Hari).
@@ -226,12 +227,6 @@ __global__ void set_shift_kernel(int n, double *A, int64_t lda, EigScalars *sc)
     if (i == 0) sc->sigma = sg;
 }
 
-__global__ void set_identity_kernel(int n, double *V, int64_t ldv)
-{
-    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e < (int64_t)n * n) { const int i = (int)(e % n), j = (int)(e / n); V[i + (int64_t)j * ldv] = (i == j) ? 1.0 : 0.0; }
-}
-
 __global__ void init_scalars_kernel(EigScalars *sc)
 {
     sc->sigma = 0.0; sc->rowsum_max = 0.0; sc->off_max = 0ull; sc->done = 0; sc->status = 0; sc->sweeps = 0; sc->pad = 0;
@@ -284,6 +279,7 @@ jacobi_round_kernel(int n, int npad, int round, double *G, int64_t ldg, double *
         gp[i] = cs * x - sn * y;
         gq[i] = sn * x + cs * y;
     }
+    if (!V) return;                                    // the rotations are recovered from G afterwards (V = G_0^-1 G)
     double *vp = V + (int64_t)p * ldv, *vq = V + (int64_t)q * ldv;
     for (int i = threadIdx.x; i < n; i += blockDim.x) {
         const double x = vp[i], y = vq[i];
@@ -428,13 +424,14 @@ extern "C" int sparc_gpu_eigensolve(sparc_gpu_ctx *ctx, int64_t n64, const doubl
     EIG_LAUNCH(0, (transpose_kernel<false><<<tg, 256, 0, st>>>(n, B2, ld, B3, ld)));
     SPARC_TRY(trsm_lower_fwd(ctx, n, n, B1, ld, B3, ld, sc, st));
     EIG_LAUNCH(0, (symmetrize_kernel<<<n, 256, 0, st>>>(n, B3, ld, B2, ld, sc)));
-    // E3: B3 <- A (kept for the Rayleigh quotients), B2 <- chol(A + sigma I), B4 = G = R^T, then B2 = V = I
+    // E3: B3 <- A (kept for the Rayleigh quotients), B2 <- R = chol(A + sigma I), B4 = G = R^T.  The product of the rotations is
+    // not accumulated (that would double the traffic of every round): G_final = G_0 V with G_0 = R^T, so V = R^-T G_final by one
+    // blocked back substitution at the end.
     SPARC_CUDA_TRY(cudaMemcpyAsync(B3, B2, (size_t)ld * n * 8, cudaMemcpyDeviceToDevice, st));
     EIG_LAUNCH(0, (set_shift_kernel<<<(n + 255) / 256, 256, 0, st>>>(n, B2, ld, sc)));
     SPARC_TRY(potrf_lower(ctx, n, B2, ld, sc, st));
     EIG_LAUNCH(0, (transpose_kernel<true><<<tg, 256, 0, st>>>(n, B2, ld, B4, ld)));
-    EIG_LAUNCH(0, (set_identity_kernel<<<(unsigned)(((int64_t)n * n + 255) / 256), 256, 0, st>>>(n, B2, ld)));
-    double *G = B4, *V = B2, *A = B3;
+    double *G = B4, *R = B2, *A = B3;
     {
         const int npad = n + (n & 1);
         const double tol = 2.3e-16 * sqrt((double)n) * 2.0;
@@ -446,23 +443,24 @@ extern "C" int sparc_gpu_eigensolve(sparc_gpu_ctx *ctx, int64_t n64, const doubl
         if (n > 1) {
             for (int sweep = 0; sweep < MAX_SWEEPS; ++sweep) {
                 for (int r = 0; r < npad - 1; ++r)
-                    EIG_LAUNCH(0, (jacobi_round_kernel<<<npad / 2, 256, smem, st>>>(n, npad, r, G, ld, V, ld, tol, sc)));
+                    EIG_LAUNCH(0, (jacobi_round_kernel<<<npad / 2, 256, smem, st>>>(n, npad, r, G, ld, nullptr, ld, tol, sc)));
                 EIG_LAUNCH(0, (sweep_end_kernel<<<1, 1, 0, st>>>(tol, sweep == MAX_SWEEPS - 1, sc)));
             }
         }
     }
-    // E4: mu = diag(V^T A V); G <- A V (G is free now)
-    SPARC_CUDA_TRY(cudaMemsetAsync(G, 0, (size_t)ld * n * 8, st));
+    SPARC_TRY(trsm_lower_trans_bwd(ctx, n, n, R, ld, G, ld, sc, st));          // G <- V = R^-T G
+    double *V = G, *W = B2;                                                      // R is no longer needed: W = scratch
+    // E4: mu = diag(V^T A V) with W = -(A V) through the subtracting kernel (the sign is undone in the quotient)
+    SPARC_CUDA_TRY(cudaMemsetAsync(W, 0, (size_t)ld * n * 8, st));
     {
         dim3 grid((n + 63) / 64, (n + 63) / 64);
-        // G = -(A V) through the subtracting kernel; the sign is undone in the quotient below
-        EIG_LAUNCH(0, (gemm_sub_kernel<false, false><<<grid, 256, 0, st>>>(n, n, n, A, ld, V, ld, G, ld, nullptr)));
+        EIG_LAUNCH(0, (gemm_sub_kernel<false, false><<<grid, 256, 0, st>>>(n, n, n, A, ld, V, ld, W, ld, nullptr)));
     }
-    EIG_LAUNCH(0, (rayleigh_kernel<<<n, 256, 0, st>>>(n, V, ld, G, ld, -1.0, mu)));
+    EIG_LAUNCH(0, (rayleigh_kernel<<<n, 256, 0, st>>>(n, V, ld, W, ld, -1.0, mu)));
     EIG_LAUNCH(0, (rank_kernel<<<(n + 255) / 256, 256, 0, st>>>(n, mu, rank, D)));
-    EIG_LAUNCH(0, (permute_cols_kernel<<<dim3((n + 255) / 256 > 8 ? 8 : (n + 255) / 256, n), 256, 0, st>>>(n, V, ld, rank, G, ld)));
-    SPARC_TRY(trsm_lower_trans_bwd(ctx, n, n, B1, ld, G, ld, sc, st));
-    SPARC_CUDA_TRY(cudaMemcpy2DAsync(Z, (size_t)n * 8, G, (size_t)ld * 8, (size_t)n * 8, (size_t)n, cudaMemcpyDeviceToDevice, st));
+    EIG_LAUNCH(0, (permute_cols_kernel<<<dim3((n + 255) / 256 > 8 ? 8 : (n + 255) / 256, n), 256, 0, st>>>(n, V, ld, rank, W, ld)));
+    SPARC_TRY(trsm_lower_trans_bwd(ctx, n, n, B1, ld, W, ld, sc, st));
+    SPARC_CUDA_TRY(cudaMemcpy2DAsync(Z, (size_t)n * 8, W, (size_t)ld * 8, (size_t)n * 8, (size_t)n, cudaMemcpyDeviceToDevice, st));
     if (info) SPARC_CUDA_TRY(cudaMemcpyAsync(info, &sc->status, 2 * sizeof(int), cudaMemcpyDeviceToDevice, st));
     return SPARC_GPU_SUCCESS;
 }
