@@ -191,3 +191,8 @@ def test_config4_fullsize_sampled(torch, api):
     if total < 150e9:
         pytest.skip("config 4 needs a 180 GB B200")
     fullsize_parity(torch, api, 4, n_random_cols=8, n_gram=10, n_random_rows=32, check_invariants=False)
+
+
+def test_config5_fullsize_sampled(torch, api):
+    """The sixth workload (128^3, h = 0.22, degree 33): the x-tiled hybrid stencil at full size."""
+    fullsize_parity(torch, api, 5, n_random_cols=4, n_gram=8, n_random_rows=32, check_invariants=True)
