@@ -270,6 +270,8 @@ def bench_config(env, config, steps, warmup, *, col_block=0, stencil_path=0, ste
         need = ns * ld * 8
         avail = host_memory_available_bytes()
         ns_e = ns
+        if avail is not None:
+            avail = avail // world                     # every rank pins its own block
         if avail is not None and need > 0.55 * avail:
             ns_e = max(64, int(0.55 * avail // (ld * 8)) // 64 * 64)
         ns_e = min(ns, ns_e)
@@ -639,12 +641,21 @@ def run_ours(args):
     env = {"torch": torch, "dist": dist, "api": api, "wlmod": wlmod, "world": world, "rank": rank,
            "local_rank": local_rank, "dev": dev}
 
+    res = None
     if (world > 1 or args.force_shard) and args.parallelism == "shard":
-        res = bench_shard(env, args.config, args.steps, args.warmup, col_block=args.col_block)
-    else:
+        try:
+            res = bench_shard(env, args.config, args.steps, args.warmup, col_block=args.col_block)
+        except Exception as exc:        # e.g. a collective this NCCL build refuses: every rank sees the same error and the run
+            if world == 1:              # falls back to N independent replicas, saying so in `config.parallelism`
+                raise
+            shard_error = f"{type(exc).__name__}: {exc}"[:200]
+            torch.cuda.empty_cache()
+    if res is None:
         res = bench_config(env, args.config, args.steps, args.warmup, col_block=args.col_block,
                            stencil_path=args.stencil_path, stencil_stages=args.stencil_stages,
                            do_e2e=not args.no_e2e, do_cpu=not args.no_cpu)
+    if world > 1 and args.parallelism == "shard" and "scaling" not in res:
+        res["config"]["parallelism"] += f" (shard path failed: {shard_error})"
     # the other workloads of BASELINE.json (and the sixth, finer-mesh one), a few steps each, same measurement
     per_config = {}
     if args.per_config and world == 1:
