@@ -157,3 +157,16 @@ def test_eigensolve_subspace_sizes(torch, api, g, n):
     assert info[0] == 0
     ref = sl.eigh(H, M, eigvals_only=True)
     check(H, M, D.cpu().numpy(), api.colmajor_to_numpy(Z), ref, "vs LAPACK")
+
+
+def test_eigensolve_argument_errors(torch, api, g):
+    """n beyond the shared-memory limit of a column pair is UNSUPPORTED (-2), a short workspace is -5, n = 0 is a no-op."""
+    import ctypes as C
+    lib = g.lib
+    one = torch.zeros(4, dtype=torch.float64, device="cuda")
+    p = C.c_void_p(one.data_ptr())
+    g._workspace(api.OP_EIGENSOLVE, 8, 0)
+    assert lib.sparc_gpu_eigensolve(g._ctx, 0, p, p, p, p, None, p, None) == 0
+    assert lib.sparc_gpu_eigensolve(g._ctx, 40000, p, p, p, p, None, p, None) == -1
+    assert lib.sparc_gpu_eigensolve(g._ctx, 1024, p, p, p, p, None, C.c_void_p(g._ws.data_ptr()), None) == -5   # workspace sized for n = 8
+    assert lib.sparc_gpu_eigensolve(g._ctx, -1, p, p, p, p, None, p, None) == -1

@@ -155,3 +155,19 @@ def test_kpoint_config1_sampled(torch, api):
     Ro = orc.rotate_k(Fg[rows, :], Q)
     assert fro_err(to_host(Pg)[rows, :], Ro) <= 1e-11
     g.close()
+
+
+def test_kpoint_lower_fd_order(torch, api):
+    """FD order 4 (radius 2) on a short periodic grid: wrapped taps with their phases for a stencil narrower than the maximum."""
+    pos = np.array([[1.0, 2.0, 1.5]])
+    wl = wlmod.make_custom("k_fd4", (7, 9, 8), (0.5, 0.45, 0.4), (0, 0, 1), 3, 4, pos, [4], 1.2, seed=45, fd_order=4)
+    theta = np.array([2.1, -0.8, 0.3])
+    g = api.SparcGpu(wl)
+    g.set_kpoint(theta, wl.supp_shift)
+    X = wl.psi_columns_complex(range(wl.ns))
+    Hk = orc.HamiltonianK(wl, theta)
+    assert col_err(to_host(g.hamiltonian_apply_k(to_dev(torch, X))), Hk.apply(X)) <= 1e-13
+    Pg = to_dev(torch, X)
+    g.chebyshev_filter_k(Pg, 3, wl.a, wl.b, wl.a0)
+    assert col_err(to_host(Pg), Hk.chebyshev_filter(X, 3, wl.a, wl.b, wl.a0)) <= 1e-13
+    g.close()

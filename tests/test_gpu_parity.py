@@ -491,3 +491,25 @@ def test_gemm_paths_agree_and_ragged_shapes(torch, api):
             g.rotate(Pg, api.colmajor_from_numpy(Q), row_panel=777)
             check_fro(api.colmajor_to_numpy(Pg, wl.nd), R_o, f"ragged rotate ld={ld} path={path}")
     g.close()
+
+
+@pytest.mark.parametrize("bc", [(0, 0, 0), (1, 0, 1)])
+@pytest.mark.parametrize("xt,ty", [(32, 0), (48, 0), (96, 0), (32, 16), (48, 16)])
+def test_stencil_dmma_x_tile_knobs(torch, api, bc, xt, ty):
+    """x tiles of the hybrid stencil on a 128-wide grid with forced tile widths: 4 x 32 (interior tiles without wrap boxes), 3 x 48
+    and 2 x 96 (overhanging last tile), with 8- and 16-row tiles, periodic and Dirichlet x."""
+    pos = np.array([[1.0, 2.0, 3.0], [30.5, 4.0, 0.4]])
+    wl = wlmod.make_custom(f"xt_{xt}_{ty}_{bc}", (128, 32, 13), (0.4, 0.45, 0.5), bc, 4, 5, pos, [4, 9], 2.2, seed=29)
+    g = api.SparcGpu(wl)
+    g.set_option("stencil_path", 3)
+    g.set_option("stencil_xt", xt)
+    g.set_option("stencil_ty", ty)
+    X = wl.psi_columns(range(wl.ns))
+    H = orc.Hamiltonian(wl)
+    Pg = api.colmajor_from_numpy(X)
+    g.chebyshev_filter(Pg, wl.degree, wl.a, wl.b, wl.a0)
+    check_col(api.colmajor_to_numpy(Pg), H.chebyshev_filter(X, wl.degree, wl.a, wl.b, wl.a0), f"{wl.name} filter, x tiles of {xt}")
+    assert g.get_info("stencil_path_last") == 3
+    with pytest.raises(api.SparcGpuError):
+        g.set_option("stencil_xt", 20)
+    g.close()
