@@ -168,5 +168,10 @@ def test_eigensolve_argument_errors(torch, api, g):
     g._workspace(api.OP_EIGENSOLVE, 8, 0)
     assert lib.sparc_gpu_eigensolve(g._ctx, 0, p, p, p, p, None, p, None) == 0
     assert lib.sparc_gpu_eigensolve(g._ctx, 40000, p, p, p, p, None, p, None) == -1
-    assert lib.sparc_gpu_eigensolve(g._ctx, 1024, p, p, p, p, None, C.c_void_p(g._ws.data_ptr()), None) == -5   # workspace sized for n = 8
     assert lib.sparc_gpu_eigensolve(g._ctx, -1, p, p, p, p, None, p, None) == -1
+    declared = g._ws.numel()
+    try:        # declare a workspace that holds n = 8 only: n = 1024 must be refused, not overrun it
+        assert lib.sparc_gpu_set_workspace_size(g._ctx, g.workspace_bytes(api.OP_EIGENSOLVE, 8)) == 0
+        assert lib.sparc_gpu_eigensolve(g._ctx, 1024, p, p, p, p, None, C.c_void_p(g._ws.data_ptr()), None) == -5
+    finally:
+        lib.sparc_gpu_set_workspace_size(g._ctx, declared)
