@@ -267,6 +267,7 @@ int sparc_gpu_probe_peak(int device, int kind, double *value_out, void *scratch_
  *   "stencil_ay" (0 auto, 1, 2), "stencil_ty" (0 auto, else tile rows), "stencil_stages" (0 auto, 2..8 TMA ring depth),
  *   "stencil_zchunks" (0 auto), "stencil_xt" (0 auto, else 32..96 multiple of 8: x-tile width of the hybrid kernel on grids
  *   wider than 96 points): tile knobs of the stencil kernels
+ *   "eig_coop"        1 (default): one cooperative launch per Jacobi sweep of sparc_gpu_eigensolve, 0: one launch per round
  *   "profile" (0 / 1), "profile_reset": per-kernel CUDA-event timing, read back through sparc_gpu_get_info */
 int sparc_gpu_set_option(sparc_gpu_ctx *ctx, const char *key, int64_t value);
 

@@ -479,6 +479,7 @@ int sparc_gpu_set_option(sparc_gpu_ctx *ctx, const char *key, int64_t value)
     if (!strcmp(key, "stencil_ty")) { if (value < 0) return SPARC_GPU_INVALID_ARG; ctx->opt_stencil_ty = (int)value; ctx->tma_choice.valid = 0; return 0; }
     // ring depth 2..8 (a one-stage ring cannot overlap the TMA copy with the arithmetic: rejected here, not at launch)
     if (!strcmp(key, "stencil_stages")) { if (value != 0 && (value < 2 || value > 8)) return SPARC_GPU_INVALID_ARG; ctx->opt_stencil_stages = (int)value; ctx->tma_choice.valid = 0; return 0; }
+    if (!strcmp(key, "eig_coop")) { ctx->opt_eig_coop = value ? 1 : 0; return 0; }
     if (!strcmp(key, "stencil_xt")) { if (value != 0 && (value < 32 || value > 96 || value % 8)) return SPARC_GPU_INVALID_ARG; ctx->opt_stencil_xt = (int)value; return 0; }
     if (!strcmp(key, "stencil_zchunks")) { if (value < 0) return SPARC_GPU_INVALID_ARG; ctx->opt_stencil_zchunks = (int)value; return 0; }
     if (!strcmp(key, "nlb_dbg")) { ctx->opt_nlb_dbg = (int)value; return 0; }

@@ -17,6 +17,8 @@
 //   E4  eigenvalues refined as Rayleigh quotients mu_j = v_j^T A v_j, sorted ascending (stable rank sort), Z = L^-T V
 //       (blocked back substitution).
 // info[0] = status: 0 ok, 1 Ms not positive definite, 2 Jacobi not converged in the sweep budget; info[1] = sweeps used.
+#include <cooperative_groups.h>
+
 #include <algorithm>
 
 #include "internal.h"
@@ -245,14 +247,12 @@ __device__ __forceinline__ double block_sum(double v, double *red)
     return s;
 }
 
-// One round of the tournament: CTA b rotates the column pair (p, q) of G and V so that g_p . g_q = 0.
-__global__ void __launch_bounds__(256)
-jacobi_round_kernel(int n, int npad, int round, double *G, int64_t ldg, double *V, int64_t ldv, double tol, EigScalars *sc)
+// One pair of one tournament round: the CTA rotates the columns (p, q) of G (and of V, if accumulated) so that g_p . g_q = 0.
+// Every thread of the CTA takes the same path (the barriers inside block_sum are uniform).
+__device__ __forceinline__ void jacobi_pair(int n, int npad, int round, int k, double *G, int64_t ldg, double *V, int64_t ldv,
+                                            double tol, EigScalars *sc, double *cols, double *red)
 {
-    if (sc->done) return;
-    extern __shared__ double cols[];                   // g_p, g_q
-    __shared__ double red[8];
-    const int m = npad - 1, k = blockIdx.x;
+    const int m = npad - 1;
     int p, q;
     if (k == 0) { p = round % m; q = npad - 1; }
     else { p = (round + k) % m; q = (round - k + m) % m; }
@@ -288,14 +288,49 @@ jacobi_round_kernel(int n, int npad, int round, double *G, int64_t ldg, double *
     }
 }
 
-__global__ void sweep_end_kernel(double tol, int last, EigScalars *sc)
+// One round per launch: CTA k takes pair k (the fallback when a cooperative launch is not possible).
+__global__ void __launch_bounds__(256)
+jacobi_round_kernel(int n, int npad, int round, double *G, int64_t ldg, double *V, int64_t ldv, double tol, EigScalars *sc)
 {
     if (sc->done) return;
+    extern __shared__ double cols[];                   // g_p, g_q
+    __shared__ double red[8];
+    jacobi_pair(n, npad, round, blockIdx.x, G, ldg, V, ldv, tol, sc, cols, red);
+}
+
+__device__ __forceinline__ void sweep_end(double tol, int last, EigScalars *sc)
+{
     sc->sweeps += 1;
     const double off = __longlong_as_double((long long)sc->off_max);
     if (off <= tol) sc->done = 1;
     else if (last) { sc->done = 1; sc->status = 2; }
     sc->off_max = 0ull;
+}
+
+// A whole sweep (n - 1 rounds) in ONE cooperative launch: the co-resident CTAs share the pairs of a round and meet at a
+// grid-wide barrier between rounds, which costs a fraction of a kernel launch -- for N_s <= 2048 the factor sits in L2 and the
+// per-round launches were the bottleneck.  `done` is read once at the start (it only changes after the last barrier).
+__global__ void __launch_bounds__(256)
+jacobi_sweep_coop_kernel(int n, int npad, double *G, int64_t ldg, double tol, int last, EigScalars *sc)
+{
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    extern __shared__ double cols[];
+    __shared__ double red[8];
+    if (sc->done) return;
+    for (int r = 0; r < npad - 1; ++r) {
+        for (int k = blockIdx.x; k < npad / 2; k += gridDim.x) {
+            jacobi_pair(n, npad, r, k, G, ldg, nullptr, 0, tol, sc, cols, red);
+            __syncthreads();                           // the staged pair is rewritten by the CTA's next pair
+        }
+        grid.sync();
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) sweep_end(tol, last, sc);
+}
+
+__global__ void sweep_end_kernel(double tol, int last, EigScalars *sc)
+{
+    if (sc->done) return;
+    sweep_end(tol, last, sc);
 }
 
 // mu[j] = sign * v_j . w_j (Rayleigh quotient v_j^T A v_j with W = sign * A V precomputed), one CTA per column
@@ -440,7 +475,26 @@ extern "C" int sparc_gpu_eigensolve(sparc_gpu_ctx *ctx, int64_t n64, const doubl
             SPARC_CUDA_TRY(cudaFuncSetAttribute(jacobi_round_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
             ctx->func_attr_done |= 1ull << 40;
         }
-        if (n > 1) {
+        if (smem > 48 * 1024 && !(ctx->func_attr_done & (1ull << 41))) {
+            SPARC_CUDA_TRY(cudaFuncSetAttribute(jacobi_sweep_coop_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+            ctx->func_attr_done |= 1ull << 41;
+        }
+        // cooperative sweeps when the device supports them and at least one CTA per SM fits
+        int coop = 0, occ = 0;
+        if (ctx->opt_eig_coop && cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, ctx->device) == cudaSuccess && coop &&
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, jacobi_sweep_coop_kernel, 256, smem) == cudaSuccess && occ >= 1) {
+            const int grid = std::min(npad / 2, occ * ctx->sm_count);
+            for (int sweep = 0; sweep < MAX_SWEEPS && n > 1; ++sweep) {
+                int nn = n, np_ = npad, last = sweep == MAX_SWEEPS - 1;
+                int64_t ldl = ld;
+                double tl = tol;
+                void *args[] = {&nn, &np_, &G, &ldl, &tl, &last, &sc};
+                prof_begin(ctx, KK_EIG, st);
+                SPARC_CUDA_TRY(cudaLaunchCooperativeKernel((const void *)jacobi_sweep_coop_kernel, dim3(grid), dim3(256), args, smem, st));
+                prof_end(ctx, KK_EIG, st);
+            }
+        } else if (n > 1) {
+            (void)cudaGetLastError();
             for (int sweep = 0; sweep < MAX_SWEEPS; ++sweep) {
                 for (int r = 0; r < npad - 1; ++r)
                     EIG_LAUNCH(0, (jacobi_round_kernel<<<npad / 2, 256, smem, st>>>(n, npad, r, G, ld, nullptr, ld, tol, sc)));

@@ -96,6 +96,7 @@ struct sparc_gpu_ctx {
     int opt_stencil_ty = 0;        // 0 auto, else forced tile rows of the TMA stencil kernel
     int opt_stencil_stages = 0;    // 0 auto, else cap on the smem ring depth (2..8)
     int opt_stencil_xt = 0;        // 0 auto, else forced x-tile width of the hybrid stencil on grids wider than 96 (32..96, multiple of 8)
+    int opt_eig_coop = 1;          // eigensolve: 1 = one cooperative launch per Jacobi sweep (grid barrier between rounds), 0 = one launch per round
     int opt_stencil_zchunks = 0;   // 0 auto, else forced number of z chunks
     // size of the buffer the caller passes as ws_dev (sparc_gpu_set_workspace_size); 0 = not declared, no check
     int64_t ws_bytes = 0;
