@@ -79,8 +79,6 @@ __device__ __forceinline__ void tma_store_4d(const CUtensorMap *tmap, uint32_t s
 }
 __device__ __forceinline__ void tma_store_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void tma_store_wait_read_all() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
-// all but the most recent bulk group of this thread have finished reading shared memory
-__device__ __forceinline__ void tma_store_wait_read_1() { asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 // global[0 .. bytes) += shared[0 .. bytes) element-wise in FP64 (UBLKRED.ADD.F64); bytes and both addresses multiples of 16
 __device__ __forceinline__ void bulk_reduce_add_f64(double *dst, uint32_t src, uint32_t bytes)
