@@ -746,10 +746,11 @@ int launch_persist(sparc_gpu_ctx *ctx, int mode, BrickParams &P, const CUtensorM
     const int cap = (int)std::max<int64_t>(B.max_blocks, NB_OCT);
     P.cap_blocks = cap;
     const size_t smem = 2048 + (size_t)NLP_WARPS * (NLP_TILE_BYTES + NLP_SLAB_BYTES) + (size_t)cap * BLK * 8;
-    // units = (brick, chunk of column groups): whole bricks when there are enough of them to balance the SMs, else chunks
-    // of at least one group per warp
+    // units = (brick, chunk of column groups): whole bricks when there are enough of them to balance the SMs (three units per
+    // SM: measured at config 1, 80 us with 582 whole-brick units against 87 us with 1164 half units -- a longer unit amortises
+    // its chi-block load and keeps the warps' tile prefetch running), else chunks of at least one group per warp
     int chunk_len = ngroups;
-    while ((int64_t)B.n_active * ((ngroups + chunk_len - 1) / chunk_len) < 6LL * ctx->sm_count && chunk_len > NLP_GSTEP)
+    while ((int64_t)B.n_active * ((ngroups + chunk_len - 1) / chunk_len) < 3LL * ctx->sm_count && chunk_len > NLP_GSTEP)
         chunk_len = std::max(NLP_GSTEP, (chunk_len / 2 + NLP_GSTEP - 1) / NLP_GSTEP * NLP_GSTEP);
     const int nchunks = (ngroups + chunk_len - 1) / chunk_len;
     const int64_t nunits = (int64_t)B.n_active * nchunks;
