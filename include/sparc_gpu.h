@@ -60,7 +60,8 @@ typedef enum {
                                            atom, inconsistent chi_ptr / supp_ptr, n_proj < 0 or > 16        */
     SPARC_GPU_WORKSPACE_TOO_SMALL = -5, /* the call needs more scratch than sparc_gpu_set_workspace_size declared */
     SPARC_GPU_OUT_OF_MEMORY = -6,       /* device allocation of the library's tables failed                 */
-    SPARC_GPU_CUDA_ERROR = -7           /* any other CUDA runtime / driver error                            */
+    SPARC_GPU_CUDA_ERROR = -7,          /* any other CUDA runtime / driver error                            */
+    SPARC_GPU_STATIC_SCRATCH_EXCEEDED = -8  /* sparc_gpu_gram_static: m * n is more than the built-in scratch holds */
 } sparc_gpu_status;
 
 typedef enum {
@@ -218,6 +219,34 @@ int sparc_gpu_gram(sparc_gpu_ctx *ctx, const double *A_dev, int64_t lda, const d
 /* X <- X Q in place on a block of `nrows` rows (ld >= nrows): sparc_gpu_rotate for a row block (workspace op ROTATE). */
 int sparc_gpu_rotate_rows(sparc_gpu_ctx *ctx, double *X_dev, int64_t ld, int64_t nrows, int64_t ns, const double *Q_dev,
                           int64_t row_panel, void *ws_dev, void *stream);
+
+/* ---- The Gram product for callers that cannot allocate device memory ------------------------------------------------------------
+ * sparc_gpu_gram wants two things a caller may be unable to give at the moment it needs X^T Y: a context (sparc_gpu_create
+ * uploads its tables with cudaMalloc) and a workspace for the split-K partial products.  Who is in that position:
+ *   - an SCF driver that has given all free HBM to its own arena for the orbital blocks (Psi of the largest workload is 82 GB;
+ *     with H Psi beside it nothing is left to lend as ws_dev), or an MPI rank under a per-process memory cap (MPS, MIG slice)
+ *     where a cudaMalloc in the middle of an SCF iteration can fail;
+ *   - code inside an overlapped region, such as the distributed step with copies, collectives and kernels in flight on several
+ *     streams: cudaFree waits for the whole device and cudaMalloc may, so either one stalls every stream;
+ *   - a plug-in inside a host application whose rules route all device memory through the host's allocator.
+ * sparc_gpu_gram_static computes the same C = A^T B (layouts, `symmetric` and the fixed-order, bitwise repeatable reduction
+ * as in sparc_gpu_gram) and calls no cudaMalloc, cudaFree or allocating library routine, ever.  It needs no context, only the
+ * device ordinal.  Its split-K partial products go to an array of SPARC_GPU_GRAM_STATIC_MAX_ELEMS doubles (16 MiB) that is
+ * compiled into the library: every GPU on which the library's code gets loaded holds those 16 MiB until the process exits.
+ *   Limit: m * n <= SPARC_GPU_GRAM_STATIC_MAX_ELEMS (e.g. 1448 x 1448); beyond it the call does nothing and returns
+ *          SPARC_GPU_STATIC_SCRATCH_EXCEEDED.  nrows is not limited.  Fewer partials fit than in a 2 GiB workspace, so for
+ *          m * n above 32768 the row split can differ from sparc_gpu_gram's: results agree to rounding, not bit for bit.
+ *   First call on a device: looks up the array's address on that GPU (cudaGetSymbolAddress) and sets kernel attributes.  Make
+ *          that first call ahead of any stream capture; a call with nrows = 0 (C is zeroed) is enough.  Thread-safe.
+ *   Sharing: there is ONE array per GPU, shared by every call from every thread.  Two calls whose kernels can overlap on the
+ *          GPU (different streams with no dependency between them) race on it and give wrong results; calls on one stream,
+ *          or ordered by events, are safe.  The array keeps whatever the last call left in it; each call overwrites every
+ *          element it later reads, so nothing has to be (or is) cleared between calls.
+ * Errors: INVALID_ARG (NULL / negative / lda, ldb < nrows / symmetric with m != n / device outside 0..63), UNSUPPORTED (device
+ * is not compute capability 10.x), STATIC_SCRATCH_EXCEEDED, CUDA_ERROR.  nrows = 0 zeroes C. */
+#define SPARC_GPU_GRAM_STATIC_MAX_ELEMS 2097152
+int sparc_gpu_gram_static(int device, const double *A_dev, int64_t lda, const double *B_dev, int64_t ldb, int64_t nrows,
+                          int64_t m, int64_t n, double *C_dev, int symmetric, void *stream);
 
 /* One whole CheFSI step -- filter, project, rotate -- for a block that lives in HOST memory (what the paper's code does
  * around every step with cublasSet/GetVector: PAPER.md:118, 128, 138, 146, 158, 166), with the PCIe copies overlapped with

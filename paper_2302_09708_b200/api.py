@@ -31,7 +31,7 @@ EXPORTS = ["sparc_gpu_create", "sparc_gpu_destroy", "sparc_gpu_set_veff", "sparc
            "sparc_gpu_rotate", "sparc_gpu_chefsi_step_host", "sparc_gpu_gradient",
            "sparc_gpu_nl_project", "sparc_gpu_gradient_project", "sparc_gpu_nonlocal_force", "sparc_gpu_eigensolve", "sparc_gpu_set_kpoint",
            "sparc_gpu_hamiltonian_apply_k", "sparc_gpu_chebyshev_filter_k", "sparc_gpu_project_k", "sparc_gpu_rotate_k",
-           "sparc_gpu_gram", "sparc_gpu_rotate_rows", "sparc_gpu_fill_uniform", "sparc_gpu_set_option", "sparc_gpu_get_info", "sparc_gpu_probe_peak",
+           "sparc_gpu_gram", "sparc_gpu_rotate_rows", "sparc_gpu_gram_static", "sparc_gpu_fill_uniform", "sparc_gpu_set_option", "sparc_gpu_get_info", "sparc_gpu_probe_peak",
            "sparc_gpu_error_string", "sparc_gpu_version"]
 
 
@@ -84,6 +84,7 @@ def load_library(build_if_missing: bool = True):
     lib.sparc_gpu_rotate_k.argtypes = [P, P, I64, I64, P, I64, P, P]
     lib.sparc_gpu_gram.argtypes = [P, P, I64, P, I64, I64, I64, I64, P, I, P, P]
     lib.sparc_gpu_rotate_rows.argtypes = [P, P, I64, I64, I64, P, I64, P, P]
+    lib.sparc_gpu_gram_static.argtypes = [I, P, I64, P, I64, I64, I64, I64, P, I, P]
     lib.sparc_gpu_fill_uniform.argtypes = [P, I64, C.c_uint64, C.c_uint64, C.c_uint64, D, D, I, P]
     lib.sparc_gpu_probe_peak.argtypes = [I, I, C.POINTER(D), P, I64, P]
     lib.sparc_gpu_set_option.argtypes = [P, C.c_char_p, I64]
@@ -146,6 +147,35 @@ def probe_peak(kind: int, device: int = 0, scratch_bytes: int = 1 << 30) -> floa
     _check(load_library().sparc_gpu_probe_peak(int(device), int(kind), C.byref(out), C.c_void_p(scratch.data_ptr()),
                                                scratch.numel(), _stream_ptr(scratch.device)), "probe_peak")
     return out.value
+
+
+GRAM_STATIC_MAX_ELEMS = 2097152       # SPARC_GPU_GRAM_STATIC_MAX_ELEMS of include/sparc_gpu.h
+
+
+def gram_static(A, B, nrows: int, symmetric: bool = False, out=None):
+    """sparc_gpu_gram_static: C = A^T B over `nrows` rows without a context, a workspace or any device allocation by the
+    library -- for callers that cannot allocate at this point (all HBM already in their own arena or under a per-process
+    cap; inside an overlapped multi-stream region that a cudaMalloc / cudaFree would stall; memory owned by a host
+    application's allocator).  The split-K partials live in a 16 MiB array built into the library, one per GPU and shared by
+    all calls: keep calls on one stream or order them with events.  m * n <= GRAM_STATIC_MAX_ELEMS, else SparcGpuError
+    (status -8).  A, B: (m, lda), (n, ldb) float64 CUDA tensors holding the column-major nrows x m / nrows x n matrices.
+    Pass `out` ((n, m), contiguous) if this wrapper must not allocate either; the first call on a device does a one-time
+    address look-up and belongs before any stream capture.  Runs on torch's current stream of A's device."""
+    torch = _torch()
+    for t in (A, B):
+        if not (t.is_cuda and t.dtype == torch.float64 and t.dim() == 2 and t.stride(1) == 1):
+            raise ValueError("gram_static: need 2-D float64 CUDA tensors (ncols, ld) contiguous along ld")
+    m, n = int(A.shape[0]), int(B.shape[0])
+    lda = int(A.stride(0)) if m > 1 else int(A.shape[1])
+    ldb = int(B.stride(0)) if n > 1 else int(B.shape[1])
+    if out is None:
+        out = torch.empty((n, m), dtype=torch.float64, device=A.device)
+    assert out.is_cuda and out.dtype == torch.float64 and out.shape == (n, m) and out.is_contiguous()
+    dev = A.device.index if A.device.index is not None else torch.cuda.current_device()
+    _check(load_library().sparc_gpu_gram_static(int(dev), C.c_void_p(A.data_ptr()), lda, C.c_void_p(B.data_ptr()), ldb,
+                                                int(nrows), m, n, C.c_void_p(out.data_ptr()), 1 if symmetric else 0,
+                                                _stream_ptr(A.device)), "gram_static")
+    return out          # (n, m) tensor holding the column-major m x n matrix
 
 
 class SparcGpu:

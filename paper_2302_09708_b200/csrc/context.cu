@@ -323,6 +323,7 @@ const char *sparc_gpu_error_string(int code)
     case SPARC_GPU_WORKSPACE_TOO_SMALL: return "workspace too small";
     case SPARC_GPU_OUT_OF_MEMORY: return "out of device memory";
     case SPARC_GPU_CUDA_ERROR: return "CUDA error";
+    case SPARC_GPU_STATIC_SCRATCH_EXCEEDED: return "m * n exceeds the built-in static scratch of sparc_gpu_gram_static (2097152 doubles)";
     default: return "unknown status";
     }
 }

@@ -7,6 +7,7 @@
 // Small-output TN products (N_s = 32, 256) are split over K across the chip and reduced in a fixed order
 // (deterministic).
 #include <algorithm>
+#include <mutex>
 
 #include "internal.h"
 
@@ -341,5 +342,123 @@ int launch_mirror_upper(sparc_gpu_ctx *ctx, double *C, int64_t ldc, int64_t n, c
     mirror_upper_kernel<<<dim3(nt, nt), 256, 0, st>>>(C, ldc, n);
     prof_end(ctx, KK_COPY2D, st);
     SPARC_CUDA_TRY(cudaGetLastError());
+    return SPARC_GPU_SUCCESS;
+}
+
+// ---- sparc_gpu_gram_static: C = A^T B for callers that cannot allocate (include/sparc_gpu.h) ------------------------------------
+// Same DMMA kernel, same fixed-order reduction and same mirror kernel as sparc_gpu_gram; what differs is where the split-K
+// partial products live (the file-scope array below instead of the caller's workspace), that no context is needed, and that
+// the split plan is limited to what the array holds.  Nothing above this line is touched by it.
+
+namespace {
+
+constexpr int64_t GRAM_STATIC_ELEMS = SPARC_GPU_GRAM_STATIC_MAX_ELEMS;      // 2 Mi doubles = 16 MiB
+
+// The scratch itself.  It is part of the library's device image: each GPU on which this library's code is loaded sets
+// 16 MiB aside for it and keeps them until the process ends, whether or not sparc_gpu_gram_static is ever called.
+// In HOST code the identifier below is only a handle for cudaGetSymbolAddress -- it is NOT a device address and must never
+// be handed to a kernel as such (the kernel would fault, or on a system where the GPU can read host memory, quietly work
+// on the wrong bytes).  gram_static_setup() asks the runtime for the real address once per device.
+static __device__ __align__(256) double g_gram_static_scratch[GRAM_STATIC_ELEMS];
+
+constexpr int GRAM_STATIC_MAX_DEVICES = 64;
+struct GramStaticDevice {
+    bool ready = false;
+    double *scratch = nullptr;      // device address of g_gram_static_scratch on this GPU
+    int sm_count = 0;
+};
+GramStaticDevice g_gram_static_device[GRAM_STATIC_MAX_DEVICES];
+std::mutex g_gram_static_mutex;
+
+// One-time set-up for `device`, which the caller has made current: resolve the array's address on this GPU, read the SM
+// count, raise the kernels' dynamic shared-memory limit.  No allocation (the array came with the module).
+int gram_static_setup(int device, GramStaticDevice *out)
+{
+    std::lock_guard<std::mutex> lock(g_gram_static_mutex);
+    GramStaticDevice &d = g_gram_static_device[device];
+    if (!d.ready) {
+        int major = 0, sms = 0;
+        SPARC_CUDA_TRY(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device));
+        if (major != 10) return SPARC_GPU_UNSUPPORTED;                       // the library holds sm_100a code only
+        SPARC_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device));
+        double *ptr = nullptr;
+        SPARC_CUDA_TRY(cudaGetSymbolAddress((void **)&ptr, g_gram_static_scratch));
+        if (!ptr) return SPARC_GPU_CUDA_ERROR;
+        const int smem = (int)smem_bytes(false, NWN_DEFAULT);
+        SPARC_CUDA_TRY(cudaFuncSetAttribute(gemm_dmma_kernel<false, true, NWN_DEFAULT>,
+                                            cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        SPARC_CUDA_TRY(cudaFuncSetAttribute(gemm_dmma_kernel<false, false, NWN_DEFAULT>,
+                                            cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        d.scratch = ptr;
+        d.sm_count = std::max(1, sms);
+        d.ready = true;
+    }
+    *out = d;
+    return SPARC_GPU_SUCCESS;
+}
+
+// plan_tn's cost model with the static array as the cap on the partial products (splits * M * N <= GRAM_STATIC_ELEMS)
+SplitPlan plan_tn_static(int sm_count, int64_t M, int64_t N, int64_t K, int64_t diag)
+{
+    const int64_t tiles = std::max<int64_t>(1, tiles_computed(M, N, diag));
+    const int64_t slots = (int64_t)sm_count * (NWN_DEFAULT == 2 ? 2 : 1);
+    const int64_t max_splits = std::max<int64_t>(1, std::min<int64_t>(64, K / (16 * BK)));
+    const int64_t cap_elems = std::min<int64_t>(GRAM_STATIC_ELEMS, 64 * M * N);
+    int64_t best_s = 1;
+    double best_cost = 1e300;
+    for (int64_t s = 1; s <= max_splits; ++s) {
+        if (s > 1 && s * M * N > cap_elems) break;
+        const int64_t waves = (tiles * s + slots - 1) / slots;
+        const double cost = (double)waves * ((double)K / (double)s + 64.0)
+                            + (s > 1 ? 0.02 * (double)s * (double)K / 64.0 / (double)std::max<int64_t>(1, tiles / 8 + 1) : 0.0);
+        if (cost < best_cost * 0.995) { best_cost = cost; best_s = s; }
+    }
+    const int64_t chunk = round_up_i64(std::max<int64_t>((K + best_s - 1) / best_s, 1), BK);
+    return {(int)std::max<int64_t>(1, (K + chunk - 1) / chunk), chunk};
+}
+
+}  // namespace
+
+extern "C" int sparc_gpu_gram_static(int device, const double *A, int64_t lda, const double *B, int64_t ldb, int64_t nrows,
+                                     int64_t m, int64_t n, double *C, int symmetric, void *stream)
+{
+    if (device < 0 || device >= GRAM_STATIC_MAX_DEVICES || nrows < 0 || m < 0 || n < 0) return SPARC_GPU_INVALID_ARG;
+    if (m == 0 || n == 0) return SPARC_GPU_SUCCESS;
+    if (!C || (symmetric && m != n)) return SPARC_GPU_INVALID_ARG;
+    if (nrows > 0 && (!A || !B || lda < nrows || ldb < nrows)) return SPARC_GPU_INVALID_ARG;
+    if (m > GRAM_STATIC_ELEMS || n > GRAM_STATIC_ELEMS || m * n > GRAM_STATIC_ELEMS) return SPARC_GPU_STATIC_SCRATCH_EXCEEDED;
+    DeviceGuard dg(device);
+    if (!dg.ok) return SPARC_GPU_CUDA_ERROR;
+    GramStaticDevice dev;
+    SPARC_TRY(gram_static_setup(device, &dev));
+    cudaStream_t st = (cudaStream_t)stream;
+    if (nrows == 0) { SPARC_CUDA_TRY(cudaMemsetAsync(C, 0, (size_t)m * n * 8, st)); return SPARC_GPU_SUCCESS; }
+
+    constexpr int BN = 32 * NWN_DEFAULT, GEMM_THREADS = 64 * NWN_DEFAULT;
+    const int64_t diag = symmetric ? 0 : -1;
+    const SplitPlan plan = plan_tn_static(dev.sm_count, m, n, nrows, diag);
+    // every partial element that the reduction reads is written by this call's GEMM launch first, so nothing in the
+    // array has to be cleared: what an earlier call left there is never read
+    double *out = plan.splits > 1 ? dev.scratch : C;
+    const int tiles_m = (int)((m + BM - 1) / BM), tiles_n = (int)((n + BN - 1) / BN);
+    const dim3 grid((unsigned)(tiles_m * tiles_n), 1, (unsigned)plan.splits);
+    const size_t smem = smem_bytes(false, NWN_DEFAULT);
+    if (aligned16(A) && aligned16(B) && lda % 2 == 0 && ldb % 2 == 0)
+        gemm_dmma_kernel<false, true, NWN_DEFAULT><<<grid, GEMM_THREADS, smem, st>>>(A, lda, B, ldb, out, m, m, n, nrows,
+                                                                                    plan.k_chunk, tiles_m, diag);
+    else
+        gemm_dmma_kernel<false, false, NWN_DEFAULT><<<grid, GEMM_THREADS, smem, st>>>(A, lda, B, ldb, out, m, m, n, nrows,
+                                                                                     plan.k_chunk, tiles_m, diag);
+    SPARC_CUDA_TRY(cudaGetLastError());
+    if (plan.splits > 1) {
+        const int64_t blocks = std::min<int64_t>((m * n + 255) / 256, (int64_t)dev.sm_count * 8);
+        splitk_reduce_kernel<<<(unsigned)blocks, 256, 0, st>>>(dev.scratch, plan.splits, m, n, C, m, diag, BN);
+        SPARC_CUDA_TRY(cudaGetLastError());
+    }
+    if (symmetric && m > 1) {
+        const unsigned nt = (unsigned)((m + 31) / 32);
+        mirror_upper_kernel<<<dim3(nt, nt), 256, 0, st>>>(C, m, m);
+        SPARC_CUDA_TRY(cudaGetLastError());
+    }
     return SPARC_GPU_SUCCESS;
 }
