@@ -174,7 +174,10 @@ int sparc_gpu_nonlocal_force(sparc_gpu_ctx *ctx, const double *Psi_dev, int64_t 
  * Z^T Ms Z = I, unique up to the sign of each column and rotations inside degenerate eigenspaces (reading R23) -- Z is the Q
  * of sparc_gpu_rotate.  Method: Cholesky Ms = L L^T, A = L^-1 Hs L^-T, one-sided Jacobi on a Cholesky factor of the shifted
  * A, Rayleigh-quotient eigenvalues, Z = L^-T V (csrc/eig.cu).  Everything is queued on `stream`; convergence is tested on the
- * device.  info_dev (2 x int32, may be NULL): [0] status 0 ok / 1 Ms not positive definite / 2 not converged, [1] sweeps.
+ * device.  info_dev (2 x int32): [0] status 0 ok / 1 Ms not positive definite / 2 not converged, [1] sweeps.  The call returns
+ * SUCCESS in all three cases (it never waits for the device): with status 1 or 2 Z and D are NOT usable, so pass info_dev and
+ * read it after synchronising -- NULL is accepted, but then a failed solve is silent.  A fixed number of sweep launches (30) is
+ * always queued; the ones after convergence return at once.
  * Workspace op EIGENSOLVE with ns = n.  n <= 12800 (a column pair must fit shared memory), else UNSUPPORTED. */
 int sparc_gpu_eigensolve(sparc_gpu_ctx *ctx, int64_t n, const double *Hs_dev, const double *Ms_dev, double *Z_dev,
                          double *D_dev, int32_t *info_dev, void *ws_dev, void *stream);
@@ -212,7 +215,8 @@ int sparc_gpu_rotate_k(sparc_gpu_ctx *ctx, double *Psi_dev, int64_t ld, int64_t 
 
 /* C (m x n, column-major, ld = m) = A^T B, contraction over `nrows` rows; A: nrows x m (lda), B: nrows x n (ldb).
  * symmetric != 0 (needs m = n and a product that IS symmetric, e.g. A = B): upper-triangle tiles + mirror (R12).
- * Workspace op GRAM with ns = max(m, n). */
+ * Workspace op GRAM with ns = max(m, n).  nrows = 0 (a rank that owns no rows): C is zeroed; A_dev, B_dev and ws_dev are not
+ * looked at and may be NULL. */
 int sparc_gpu_gram(sparc_gpu_ctx *ctx, const double *A_dev, int64_t lda, const double *B_dev, int64_t ldb, int64_t nrows,
                    int64_t m, int64_t n, double *C_dev, int symmetric, void *ws_dev, void *stream);
 
@@ -260,11 +264,25 @@ int sparc_gpu_gram_static(int device, const double *A_dev, int64_t lda, const do
  *                               sparc_gpu_eigensolve on the device or the separate operator calls)
  *   Psi_dev  : DEVICE scratch for the block, N_d x ns with ld_dev >= N_d;  mats_dev: DEVICE scratch of 3 ns^2 doubles
  *   ws_dev   : DEVICE scratch of max(workspace_bytes(CHEBYSHEV_FILTER), workspace_bytes(PROJECT), workspace_bytes(ROTATE))
- * Work is queued on `stream` and two copy streams owned by the context; the call SYNCHRONISES all three before it returns. */
+ * Work is queued on `stream` and two copy streams owned by the context; the call SYNCHRONISES all three before it returns,
+ * on success and on every error return alike (nothing is left in flight into the caller's buffers). */
 int sparc_gpu_chefsi_step_host(sparc_gpu_ctx *ctx, const double *Psi_in_host, double *Psi_out_host, int64_t ld_host,
                                int64_t ns, int degree, double a, double b, double a0, const double *Q_host,
                                double *Hs_host, double *Ms_host, double *Psi_dev, int64_t ld_dev, double *mats_dev,
                                int64_t col_block, int64_t row_panel, void *ws_dev, void *stream);
+
+/* The same step with the subspace eigenproblem inside it -- Algorithm 1 as the paper states it (filter,
+ * project, "Subspace diagonalization", rotate): after the projection Hs Z = Ms Z D is solved on the device (sparc_gpu_eigensolve,
+ * no host LAPACK in between) and the block is rotated by Z.  Differences from sparc_gpu_chefsi_step_host:
+ *   D_host (out, ns doubles, ascending), info_host (out, 2 x int32: [0] status 0 ok / 1 Ms not positive definite / 2 Jacobi not
+ *   converged, [1] sweeps) replace Q_host.  The host waits once mid-step for info.  Status 1: the block is NOT rotated,
+ *   Psi_out_host receives the filtered block and the call still returns SUCCESS -- check info_host[0].
+ *   mats_dev : 3 ns^2 + ns + 1 doubles (Hs, Ms, Z, then D and info);
+ *   ws_dev   : additionally >= workspace_bytes(EIGENSOLVE, ns).  ns is bounded as in sparc_gpu_eigensolve. */
+int sparc_gpu_chefsi_step_host_solve(sparc_gpu_ctx *ctx, const double *Psi_in_host, double *Psi_out_host, int64_t ld_host,
+                                     int64_t ns, int degree, double a, double b, double a0, double *D_host, int32_t *info_host,
+                                     double *Hs_host, double *Ms_host, double *Psi_dev, int64_t ld_dev, double *mats_dev,
+                                     int64_t col_block, int64_t row_panel, void *ws_dev, void *stream);
 
 /* ---- support entry points (not operators of the method) ------------------------------------- */
 

@@ -28,7 +28,7 @@ OP_GRAM = 11
 EXPORTS = ["sparc_gpu_create", "sparc_gpu_destroy", "sparc_gpu_set_veff", "sparc_gpu_workspace_bytes",
            "sparc_gpu_set_workspace_size",
            "sparc_gpu_hamiltonian_apply", "sparc_gpu_chebyshev_filter", "sparc_gpu_project",
-           "sparc_gpu_rotate", "sparc_gpu_chefsi_step_host", "sparc_gpu_gradient",
+           "sparc_gpu_rotate", "sparc_gpu_chefsi_step_host", "sparc_gpu_chefsi_step_host_solve", "sparc_gpu_gradient",
            "sparc_gpu_nl_project", "sparc_gpu_gradient_project", "sparc_gpu_nonlocal_force", "sparc_gpu_eigensolve", "sparc_gpu_set_kpoint",
            "sparc_gpu_hamiltonian_apply_k", "sparc_gpu_chebyshev_filter_k", "sparc_gpu_project_k", "sparc_gpu_rotate_k",
            "sparc_gpu_gram", "sparc_gpu_rotate_rows", "sparc_gpu_gram_static", "sparc_gpu_fill_uniform", "sparc_gpu_set_option", "sparc_gpu_get_info", "sparc_gpu_probe_peak",
@@ -72,6 +72,7 @@ def load_library(build_if_missing: bool = True):
     lib.sparc_gpu_project.argtypes = [P, P, I64, I64, P, P, I64, P, P]
     lib.sparc_gpu_rotate.argtypes = [P, P, I64, I64, P, I64, P, P]
     lib.sparc_gpu_chefsi_step_host.argtypes = [P, P, P, I64, I64, I, D, D, D, P, P, P, P, I64, P, I64, I64, P, P]
+    lib.sparc_gpu_chefsi_step_host_solve.argtypes = [P, P, P, I64, I64, I, D, D, D, P, P, P, P, P, I64, P, I64, I64, P, P]
     lib.sparc_gpu_gradient.argtypes = [P, I, P, I64, P, I64, I64, P]
     lib.sparc_gpu_nl_project.argtypes = [P, P, I64, I64, P, P]
     lib.sparc_gpu_gradient_project.argtypes = [P, I, P, I64, I64, P, I64, P, P]
@@ -371,6 +372,38 @@ class SparcGpu:
             C.c_void_p(Ms_host.data_ptr()), pp, ldd, C.c_void_p(mats_dev.data_ptr()), int(col_block), int(row_panel),
             C.c_void_p(self._ws.data_ptr()), self._stream()), "chefsi_step_host")
         return host_out
+
+    def chefsi_step_host_solve(self, host_psi, Hs_host, Ms_host, degree: int, a: float, b: float, a0: float,
+                               psi_dev=None, mats_dev=None, col_block: int = 0, row_panel: int = 0, host_out=None):
+        """sparc_gpu_chefsi_step_host_solve: filter -> project -> device eigensolve -> rotate on a block in (pinned) HOST
+        memory (Algorithm 1 with no caller-supplied Q).  Returns (host_out, D (ns,) CPU tensor, info (2,) int32 CPU tensor)."""
+        torch = _torch()
+        ns, ld = int(host_psi.shape[0]), int(host_psi.shape[1])
+        host_out = host_psi if host_out is None else host_out
+        for t in (host_psi, host_out, Hs_host, Ms_host):
+            assert (not t.is_cuda) and t.dtype == torch.float64 and t.is_contiguous()
+        assert ld >= self.nd and host_out.shape == host_psi.shape
+        dev = torch.device("cuda", self.device)
+        if psi_dev is None:
+            psi_dev = torch.empty((ns, self.nd), dtype=torch.float64, device=dev)
+        if mats_dev is None:
+            mats_dev = torch.empty(3 * ns * ns + ns + 1, dtype=torch.float64, device=dev)
+        assert mats_dev.numel() >= 3 * ns * ns + ns + 1
+        pp, ldd, _ = self._mat(psi_dev, "psi_dev")
+        need = max(self.workspace_bytes(OP_CHEBYSHEV_FILTER, ns, col_block), self.workspace_bytes(OP_PROJECT, ns, col_block),
+                   self.workspace_bytes(OP_ROTATE, ns, row_panel), self.workspace_bytes(OP_EIGENSOLVE, ns, 0))
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = None
+            self._ws = torch.empty(need, dtype=torch.uint8, device=dev)
+            _check(self.lib.sparc_gpu_set_workspace_size(self._ctx, self._ws.numel()), "set_workspace_size")
+        D = torch.empty(ns, dtype=torch.float64).pin_memory()
+        info = torch.zeros(2, dtype=torch.int32).pin_memory()
+        _check(self.lib.sparc_gpu_chefsi_step_host_solve(
+            self._ctx, C.c_void_p(host_psi.data_ptr()), C.c_void_p(host_out.data_ptr()), ld, ns, int(degree), float(a),
+            float(b), float(a0), C.c_void_p(D.data_ptr()), C.c_void_p(info.data_ptr()), C.c_void_p(Hs_host.data_ptr()),
+            C.c_void_p(Ms_host.data_ptr()), pp, ldd, C.c_void_p(mats_dev.data_ptr()), int(col_block), int(row_panel),
+            C.c_void_p(self._ws.data_ptr()), self._stream()), "chefsi_step_host_solve")
+        return host_out, D, info
 
     # ---- NEXT-3: gradient stencil, projector contraction, nonlocal force --------------------------
     def gradient(self, X, axis: int, Y=None):

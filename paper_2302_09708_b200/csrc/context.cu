@@ -666,14 +666,17 @@ int sparc_gpu_gram(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const doubl
 {
     if (!ctx || nrows < 0 || m < 0 || n < 0) return SPARC_GPU_INVALID_ARG;
     if (m == 0 || n == 0) return SPARC_GPU_SUCCESS;
-    if (!A || !B || !C || !ws || lda < nrows || ldb < nrows || (symmetric && m != n)) return SPARC_GPU_INVALID_ARG;
+    if (!C || (symmetric && m != n)) return SPARC_GPU_INVALID_ARG;
     DeviceGuard dg(ctx->device);
     if (!dg.ok) return SPARC_GPU_CUDA_ERROR;
     cudaStream_t st = (cudaStream_t)stream;
+    // a rank that owns no rows passes empty blocks (NULL data pointers, no workspace): its contribution is C = 0, as
+    // sparc_gpu_rotate_rows treats nrows = 0 as a no-op
+    if (nrows == 0) { SPARC_CUDA_TRY(cudaMemsetAsync(C, 0, (size_t)m * n * 8, st)); return SPARC_GPU_SUCCESS; }
+    if (!A || !B || !ws || lda < nrows || ldb < nrows) return SPARC_GPU_INVALID_ARG;
     WsLayout L;
     SPARC_TRY(ws_layout(ctx, SPARC_GPU_OP_GRAM, std::max(m, n), 0, &L));
     SPARC_TRY(ws_check(ctx, L));
-    if (nrows == 0) { SPARC_CUDA_TRY(cudaMemsetAsync(C, 0, (size_t)m * n * 8, st)); return SPARC_GPU_SUCCESS; }
     const bool sym = symmetric && ctx->opt_gemm_full == 0;
     SPARC_TRY(launch_gemm_tn(ctx, A, lda, B, ldb, C, m, m, n, nrows, (char *)ws + L.off_g, sym ? 0 : -1, st));
     if (sym) SPARC_TRY(launch_mirror_upper(ctx, C, m, m, st));

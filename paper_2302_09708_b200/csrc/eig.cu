@@ -431,8 +431,9 @@ int trsm_lower_trans_bwd(sparc_gpu_ctx *ctx, int n, int nrhs, const double *L, i
 extern "C" int sparc_gpu_eigensolve(sparc_gpu_ctx *ctx, int64_t n64, const double *Hs, const double *Ms, double *Z, double *D,
                                     int32_t *info, void *ws, void *stream)
 {
-    if (!ctx || n64 < 0 || n64 > 32768) return SPARC_GPU_INVALID_ARG;
+    if (!ctx || n64 < 0) return SPARC_GPU_INVALID_ARG;
     if (n64 == 0) return SPARC_GPU_SUCCESS;
+    if (n64 > 12800) return SPARC_GPU_UNSUPPORTED;      // a column pair (2 n doubles) must fit 200 KB of shared memory
     if (!Hs || !Ms || !Z || !D || !ws) return SPARC_GPU_INVALID_ARG;
     DeviceGuard dg(ctx->device);
     if (!dg.ok) return SPARC_GPU_CUDA_ERROR;
@@ -446,7 +447,6 @@ extern "C" int sparc_gpu_eigensolve(sparc_gpu_ctx *ctx, int64_t n64, const doubl
     double *mu = B4 + ld * ld;                          // [ld]
     int *rank = (int *)(mu + ld);                       // [ld] ints
     EigScalars *sc = (EigScalars *)(mu + 2 * ld);
-    if ((size_t)2 * n * sizeof(double) > 200 * 1024) return SPARC_GPU_UNSUPPORTED;     // the column pair must fit shared memory
 
     EIG_LAUNCH(0, (init_scalars_kernel<<<1, 1, 0, st>>>(sc)));
     // E1: B1 = L

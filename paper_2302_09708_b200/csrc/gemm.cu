@@ -268,14 +268,22 @@ int launch_dmma(sparc_gpu_ctx *ctx, const double *A, int64_t lda, const double *
         const int64_t computed = tiles_computed(M, N, diag);
         ctx->gemm_flop[A_MMAJOR ? 1 : 0] += 2.0 * (double)K * (double)(BM * BN) * (double)computed;
     }
+    // the dynamic shared-memory attribute is set once per context and kernel variant (bits 42..45 of func_attr_done)
+    const uint64_t attr_bit = 1ull << (42 + (A_MMAJOR ? 2 : 0) + (vec ? 1 : 0));
     if (vec) {
         auto kern = gemm_dmma_kernel<A_MMAJOR, true, NWN>;
-        SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        if (!(ctx->func_attr_done & attr_bit)) {
+            SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            ctx->func_attr_done |= attr_bit;
+        }
         prof_begin(ctx, kind, st);
         kern<<<grid, GEMM_THREADS, smem, st>>>(A, lda, B, ldb, C, ldc, M, N, K, plan.k_chunk, tiles_m, diag);
     } else {
         auto kern = gemm_dmma_kernel<A_MMAJOR, false, NWN>;
-        SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        if (!(ctx->func_attr_done & attr_bit)) {
+            SPARC_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            ctx->func_attr_done |= attr_bit;
+        }
         prof_begin(ctx, kind, st);
         kern<<<grid, GEMM_THREADS, smem, st>>>(A, lda, B, ldb, C, ldc, M, N, K, plan.k_chunk, tiles_m, diag);
     }

@@ -339,33 +339,45 @@ int sparc_gpu_set_kpoint(sparc_gpu_ctx *ctx, const double *theta, const int8_t *
     for (int a = 0; a < 3; ++a) if (!std::isfinite(theta[a])) return SPARC_GPU_INVALID_ARG;
     DeviceGuard dg(ctx->device);
     if (!dg.ok) return SPARC_GPU_CUDA_ERROR;
-    SPARC_CUDA_TRY(cudaDeviceSynchronize());             // a previous k-point's tables may still be in use
-    for (int a = 0; a < 3; ++a) ctx->k_theta[a] = ctx->bc[a] == 0 ? theta[a] : 0.0;
-    kpoint_free(ctx);
-    ctx->k_set = 1;
-    if (ctx->supp_total == 0) return SPARC_GPU_SUCCESS;
+    // validate and build the new tables on the host FIRST: a bad shift leaves the previous k-point fully in place
+    if (supp_shift)
+        for (int64_t t = 0; t < 3 * ctx->supp_total; ++t)
+            if (supp_shift[t] < -1 || supp_shift[t] > 1) return SPARC_GPU_BAD_DESCRIPTOR;
+    double th[3];
+    for (int a = 0; a < 3; ++a) th[a] = ctx->bc[a] == 0 ? theta[a] : 0.0;
     // exp(+i phi_t) per support row, and the same numbers in the order of the point -> (atom, row) cover entries
-    std::vector<double> ph((size_t)ctx->supp_total * 2);
+    std::vector<double> ph((size_t)ctx->supp_total * 2), cph((size_t)ctx->supp_total * 2);
     for (int64_t t = 0; t < ctx->supp_total; ++t) {
         double phi = 0.0;
-        if (supp_shift) {
-            for (int a = 0; a < 3; ++a) {
-                const int w = supp_shift[3 * t + a];
-                if (w < -1 || w > 1) return SPARC_GPU_BAD_DESCRIPTOR;
-                phi += w * ctx->k_theta[a];
-            }
-        }
+        if (supp_shift)
+            for (int a = 0; a < 3; ++a) phi += supp_shift[3 * t + a] * th[a];
         ph[2 * t] = cos(phi); ph[2 * t + 1] = sin(phi);
     }
-    std::vector<double> cph((size_t)ctx->supp_total * 2);
     for (int64_t e = 0; e < ctx->supp_total; ++e) {
         const int64_t t = ctx->h_cov_row[(size_t)e];
         cph[2 * e] = ph[2 * t]; cph[2 * e + 1] = ph[2 * t + 1];
     }
-    SPARC_CUDA_TRY(cudaMalloc((void **)&ctx->d_k_phase, ph.size() * 8));
-    SPARC_CUDA_TRY(cudaMalloc((void **)&ctx->d_k_cov_phase, cph.size() * 8));
-    SPARC_CUDA_TRY(cudaMemcpy(ctx->d_k_phase, ph.data(), ph.size() * 8, cudaMemcpyHostToDevice));
-    SPARC_CUDA_TRY(cudaMemcpy(ctx->d_k_cov_phase, cph.data(), cph.size() * 8, cudaMemcpyHostToDevice));
+    SPARC_CUDA_TRY(cudaDeviceSynchronize());             // a previous k-point's tables may still be in use
+    // from here on the old k-point is gone; k_set goes back to 1 only once BOTH new tables are on the device, so that a failed
+    // upload can never leave *_k calls with k_set = 1 and NULL tables
+    ctx->k_set = 0;
+    kpoint_free(ctx);
+    for (int a = 0; a < 3; ++a) ctx->k_theta[a] = th[a];
+    if (ctx->supp_total > 0) {
+        double2 *p0 = nullptr, *p1 = nullptr;
+        cudaError_t e = cudaMalloc((void **)&p0, ph.size() * 8);
+        if (e == cudaSuccess) e = cudaMalloc((void **)&p1, cph.size() * 8);
+        if (e == cudaSuccess) e = cudaMemcpy(p0, ph.data(), ph.size() * 8, cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemcpy(p1, cph.data(), cph.size() * 8, cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) {
+            (void)cudaGetLastError();
+            cudaFree(p0); cudaFree(p1);
+            return e == cudaErrorMemoryAllocation ? SPARC_GPU_OUT_OF_MEMORY : SPARC_GPU_CUDA_ERROR;
+        }
+        ctx->d_k_phase = p0;
+        ctx->d_k_cov_phase = p1;
+    }
+    ctx->k_set = 1;
     return SPARC_GPU_SUCCESS;
 }
 

@@ -27,31 +27,45 @@ struct EventPool {
     }
 };
 
-}  // namespace
+// Whatever way the call ends, nothing of it is still in flight afterwards: an early error return would otherwise leave
+// async copies into the caller's host buffers (and kernels on three streams) running while the events are destroyed.
+struct SyncOnExit {
+    cudaStream_t s[3];
+    ~SyncOnExit() { for (auto q : s) if (cudaStreamSynchronize(q) != cudaSuccess) (void)cudaGetLastError(); }
+};
 
-extern "C" int sparc_gpu_chefsi_step_host(sparc_gpu_ctx *ctx, const double *Psi_in_host, double *Psi_out_host,
-                                          int64_t ld_host, int64_t ns, int degree, double a, double b, double a0,
-                                          const double *Q_host, double *Hs_host, double *Ms_host, double *Psi_dev,
-                                          int64_t ld_dev, double *mats_dev, int64_t col_block, int64_t row_panel,
-                                          void *ws_dev, void *stream)
+// Q_host != NULL: rotate by the caller's Q.  Q_host == NULL: Algorithm 1 as written -- the subspace
+// eigenproblem Hs Z = Ms Z D is solved on the device between projection and rotation, D and info go to the host.
+int step_host_impl(sparc_gpu_ctx *ctx, const double *Psi_in_host, double *Psi_out_host, int64_t ld_host, int64_t ns, int degree,
+                   double a, double b, double a0, const double *Q_host, double *D_host, int32_t *info_host, double *Hs_host,
+                   double *Ms_host, double *Psi_dev, int64_t ld_dev, double *mats_dev, int64_t col_block, int64_t row_panel,
+                   void *ws_dev, void *stream)
 {
+    const bool solve = Q_host == nullptr;
     if (!ctx || ns < 0 || degree < 0) return SPARC_GPU_INVALID_ARG;
     if (!(a0 < a && a < b)) return SPARC_GPU_BAD_BOUNDS;
     if (ns == 0) return SPARC_GPU_SUCCESS;
-    if (!Psi_in_host || !Psi_out_host || !Q_host || !Hs_host || !Ms_host || !Psi_dev || !mats_dev || !ws_dev ||
-        ld_host < ctx->nd || ld_dev < ctx->nd)
+    if (!Psi_in_host || !Psi_out_host || !Hs_host || !Ms_host || !Psi_dev || !mats_dev || !ws_dev ||
+        ld_host < ctx->nd || ld_dev < ctx->nd || (solve && (!D_host || !info_host)))
         return SPARC_GPU_INVALID_ARG;
     DeviceGuard dg(ctx->device);
     if (!dg.ok) return SPARC_GPU_CUDA_ERROR;
     cudaStream_t st = (cudaStream_t)stream;
-    if (!ctx->copy_stream[0]) {
-        for (int k = 0; k < 2; ++k)
-            SPARC_CUDA_TRY(cudaStreamCreateWithFlags(&ctx->copy_stream[k], cudaStreamNonBlocking));
+    if (!ctx->copy_stream[0] || !ctx->copy_stream[1]) {          // both or neither: a half-made pair is never kept
+        cudaStream_t s0 = nullptr, s1 = nullptr;
+        SPARC_CUDA_TRY(cudaStreamCreateWithFlags(&s0, cudaStreamNonBlocking));
+        const cudaError_t e1 = cudaStreamCreateWithFlags(&s1, cudaStreamNonBlocking);
+        if (e1 != cudaSuccess) { (void)cudaGetLastError(); (void)cudaStreamDestroy(s0); return SPARC_GPU_CUDA_ERROR; }
+        ctx->copy_stream[0] = s0;
+        ctx->copy_stream[1] = s1;
     }
     cudaStream_t s_in = ctx->copy_stream[0], s_out = ctx->copy_stream[1];
-    EventPool pool;
+    EventPool pool;                      // destroyed after `drain` below has synchronised the three streams
+    SyncOnExit drain{{st, s_in, s_out}};
     const int64_t nd = ctx->nd;
     double *Hs_dev = mats_dev, *Ms_dev = mats_dev + ns * ns, *Q_dev = mats_dev + 2 * ns * ns;
+    double *D_dev = mats_dev + 3 * ns * ns;                      // solve only: D[ns], then 2 x int32 info
+    int32_t *info_dev = (int32_t *)(D_dev + ns);
 
     // the copy streams start after whatever the caller queued on `stream`
     cudaEvent_t ev0 = pool.get();
@@ -79,11 +93,13 @@ extern "C" int sparc_gpu_chefsi_step_host(sparc_gpu_ctx *ctx, const double *Psi_
         SPARC_CUDA_TRY(cudaStreamWaitEvent(st, e, 0));
         SPARC_TRY(sparc_gpu_chebyshev_filter(ctx, Psi_dev + j0 * ld_dev, ld_dev, nb, degree, a, b, a0, col_block, ws_dev, st));
     }
-    // Q rides behind the columns
-    SPARC_CUDA_TRY(cudaMemcpyAsync(Q_dev, Q_host, (size_t)ns * ns * 8, cudaMemcpyHostToDevice, s_in));
-    cudaEvent_t ev_q = pool.get();
-    if (!ev_q) return SPARC_GPU_CUDA_ERROR;
-    SPARC_CUDA_TRY(cudaEventRecord(ev_q, s_in));
+    cudaEvent_t ev_q = nullptr;
+    if (!solve) {                        // Q rides behind the columns
+        SPARC_CUDA_TRY(cudaMemcpyAsync(Q_dev, Q_host, (size_t)ns * ns * 8, cudaMemcpyHostToDevice, s_in));
+        ev_q = pool.get();
+        if (!ev_q) return SPARC_GPU_CUDA_ERROR;
+        SPARC_CUDA_TRY(cudaEventRecord(ev_q, s_in));
+    }
 
     // ---- project; Hs, Ms out -----------------------------------------------------------------------------------------
     SPARC_TRY(sparc_gpu_project(ctx, Psi_dev, ld_dev, ns, Hs_dev, Ms_dev, col_block, ws_dev, st));
@@ -94,13 +110,29 @@ extern "C" int sparc_gpu_chefsi_step_host(sparc_gpu_ctx *ctx, const double *Psi_
     SPARC_CUDA_TRY(cudaMemcpyAsync(Hs_host, Hs_dev, (size_t)ns * ns * 8, cudaMemcpyDeviceToHost, s_out));
     SPARC_CUDA_TRY(cudaMemcpyAsync(Ms_host, Ms_dev, (size_t)ns * ns * 8, cudaMemcpyDeviceToHost, s_out));
 
+    // ---- solve (Q_host == NULL): Z -> Q_dev, D and info -> host; the one point where the host waits mid-step, because a
+    // pencil whose Ms is not positive definite must not be rotated by what the solver left in Z
+    bool rotate = true;
+    if (solve) {
+        SPARC_TRY(sparc_gpu_eigensolve(ctx, ns, Hs_dev, Ms_dev, Q_dev, D_dev, info_dev, ws_dev, st));
+        cudaEvent_t ev_s = pool.get();
+        if (!ev_s) return SPARC_GPU_CUDA_ERROR;
+        SPARC_CUDA_TRY(cudaEventRecord(ev_s, st));
+        SPARC_CUDA_TRY(cudaStreamWaitEvent(s_out, ev_s, 0));
+        SPARC_CUDA_TRY(cudaMemcpyAsync(D_host, D_dev, (size_t)ns * 8, cudaMemcpyDeviceToHost, s_out));
+        SPARC_CUDA_TRY(cudaMemcpyAsync(info_host, info_dev, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, s_out));
+        SPARC_CUDA_TRY(cudaStreamSynchronize(s_out));
+        rotate = info_host[0] != 1;
+    } else {
+        SPARC_CUDA_TRY(cudaStreamWaitEvent(st, ev_q, 0));
+    }
+
     // ---- rotate by row panels; finished rows out -----------------------------------------------------------------------
-    SPARC_CUDA_TRY(cudaStreamWaitEvent(st, ev_q, 0));
     int64_t rp = 0, ldw = 0;
     SPARC_TRY(rotate_layout(ctx, ns, row_panel, &rp, &ldw));
     for (int64_t r0 = 0; r0 < nd; r0 += rp) {
         const int64_t nr = std::min(rp, nd - r0);
-        SPARC_TRY(rotate_panel(ctx, Psi_dev + r0, ld_dev, nr, ns, Q_dev, (double *)ws_dev, ldw, st));
+        if (rotate) SPARC_TRY(rotate_panel(ctx, Psi_dev + r0, ld_dev, nr, ns, Q_dev, (double *)ws_dev, ldw, st));
         cudaEvent_t e = pool.get();
         if (!e) return SPARC_GPU_CUDA_ERROR;
         SPARC_CUDA_TRY(cudaEventRecord(e, st));
@@ -112,4 +144,27 @@ extern "C" int sparc_gpu_chefsi_step_host(sparc_gpu_ctx *ctx, const double *Psi_
     SPARC_CUDA_TRY(cudaStreamSynchronize(s_in));
     SPARC_CUDA_TRY(cudaStreamSynchronize(st));
     return SPARC_GPU_SUCCESS;
+}
+
+}  // namespace
+
+extern "C" int sparc_gpu_chefsi_step_host(sparc_gpu_ctx *ctx, const double *Psi_in_host, double *Psi_out_host,
+                                          int64_t ld_host, int64_t ns, int degree, double a, double b, double a0,
+                                          const double *Q_host, double *Hs_host, double *Ms_host, double *Psi_dev,
+                                          int64_t ld_dev, double *mats_dev, int64_t col_block, int64_t row_panel,
+                                          void *ws_dev, void *stream)
+{
+    if (ns > 0 && !Q_host) return SPARC_GPU_INVALID_ARG;        // the solving variant is sparc_gpu_chefsi_step_host_solve
+    return step_host_impl(ctx, Psi_in_host, Psi_out_host, ld_host, ns, degree, a, b, a0, Q_host, nullptr, nullptr, Hs_host,
+                          Ms_host, Psi_dev, ld_dev, mats_dev, col_block, row_panel, ws_dev, stream);
+}
+
+extern "C" int sparc_gpu_chefsi_step_host_solve(sparc_gpu_ctx *ctx, const double *Psi_in_host, double *Psi_out_host,
+                                                int64_t ld_host, int64_t ns, int degree, double a, double b, double a0,
+                                                double *D_host, int32_t *info_host, double *Hs_host, double *Ms_host,
+                                                double *Psi_dev, int64_t ld_dev, double *mats_dev, int64_t col_block,
+                                                int64_t row_panel, void *ws_dev, void *stream)
+{
+    return step_host_impl(ctx, Psi_in_host, Psi_out_host, ld_host, ns, degree, a, b, a0, nullptr, D_host, info_host, Hs_host,
+                          Ms_host, Psi_dev, ld_dev, mats_dev, col_block, row_panel, ws_dev, stream);
 }

@@ -100,4 +100,14 @@ def test_gram_and_rotate_rows_entry_points(torch, api):
     assert fro(api.colmajor_to_numpy(Ad, nr), orc.rotate(A, Q)) <= 1e-13
     with pytest.raises(api.SparcGpuError):
         g.gram(Ad, Bd, nr, symmetric=True)           # symmetric needs m = n
+    # a rank that owns no rows: empty blocks (NULL data pointers), no workspace -> C = 0, through the C ABI itself
+    import ctypes as C
+    Cz = torch.full((n, m), 3.0, dtype=torch.float64, device="cuda:0")
+    null = C.c_void_p(0)
+    rc = g.lib.sparc_gpu_gram(g._ctx, null, 0, null, 0, 0, m, n, C.c_void_p(Cz.data_ptr()), 0, null,
+                              C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    torch.cuda.synchronize()
+    assert rc == 0 and float(Cz.abs().max()) == 0.0
+    E = torch.empty((m, 0), dtype=torch.float64, device="cuda:0")
+    assert float(g.gram(E, E, 0, symmetric=True).abs().max()) == 0.0
     g.close()

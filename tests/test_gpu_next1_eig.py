@@ -167,7 +167,8 @@ def test_eigensolve_argument_errors(torch, api, g):
     p = C.c_void_p(one.data_ptr())
     g._workspace(api.OP_EIGENSOLVE, 8, 0)
     assert lib.sparc_gpu_eigensolve(g._ctx, 0, p, p, p, p, None, p, None) == 0
-    assert lib.sparc_gpu_eigensolve(g._ctx, 40000, p, p, p, p, None, p, None) == -1
+    assert lib.sparc_gpu_eigensolve(g._ctx, 40000, p, p, p, p, None, p, None) == -2
+    assert lib.sparc_gpu_eigensolve(g._ctx, 12801, p, p, p, p, None, p, None) == -2
     assert lib.sparc_gpu_eigensolve(g._ctx, -1, p, p, p, p, None, p, None) == -1
     declared = g._ws.numel()
     try:        # declare a workspace that holds n = 8 only: n = 1024 must be refused, not overrun it

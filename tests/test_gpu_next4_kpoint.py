@@ -115,6 +115,14 @@ def test_gamma_point_limit_and_kpoint_switch(torch, api):
     Xc = wl.psi_columns_complex(range(3))
     Y1 = to_host(g.hamiltonian_apply_k(to_dev(torch, Xc)))
     assert col_err(Y1, orc.HamiltonianK(wl, theta).apply(Xc)) <= 1e-13
+    # a set_kpoint that fails validation (image shift outside -1..1) leaves the previous k-point fully in place
+    bad = np.array(wl.supp_shift, dtype=np.int8).copy()
+    bad[-1, 2] = 2
+    with pytest.raises(api.SparcGpuError) as ei:
+        g.set_kpoint((0.2, 0.2, 0.2), bad)
+    assert ei.value.code == -4
+    Y2 = to_host(g.hamiltonian_apply_k(to_dev(torch, Xc)))
+    assert np.array_equal(Y1, Y2)
     # calls before any set_kpoint are refused
     g2 = api.SparcGpu(wl)
     with pytest.raises(api.SparcGpuError) as ei:
