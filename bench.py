@@ -356,6 +356,27 @@ def bench_config(env, config, steps, warmup, *, col_block=0, stencil_path=0, ste
                "what": "whole step filter+project+rotate through sparc_gpu_chefsi_step_host (C ABI, pinned host buffers, copies "
                        "overlapped, wall clock incl. final sync); subspace solve excluded (Q given); value = Nd*Ns*degree / step_s"
                        + ("" if ns_e == ns else f"; host memory bounds the sample to the first {ns_e} of {ns} columns")}
+        # the same step with the subspace eigenproblem inside it (Algorithm 1 whole: sparc_gpu_chefsi_step_host_solve), where the
+        # device eigensolver is in its range (one-sided Jacobi is HBM-bound past N_s ~ 2048: DESIGN.md section 6.4)
+        if ns_e == ns and ns <= 2048:
+            mats_s = torch.empty(3 * ns * ns + ns + 1, dtype=torch.float64, device=dev)
+            ts, info = [], None
+            for i in range(1 + e2e_reps):
+                refill()
+                host_psi.copy_(host_src)
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                _, _, info = g.chefsi_step_host_solve(host_psi, Hs_host, Ms_host, m, wl.a, wl.b, wl.a0, psi_dev=psi, mats_dev=mats_s,
+                                                      col_block=col_block)
+                if i > 0:
+                    ts.append(time.perf_counter() - t0)
+            tsv = torch.tensor([sum(ts) / len(ts)], dtype=torch.float64, device=dev)
+            if world > 1:
+                dist.all_reduce(tsv, op=dist.ReduceOp.MAX)
+            s_s = float(tsv.cpu()[0])
+            e2e["with_solve"] = {"value": float(nd) * ns * m * world / s_s, "step_s": s_s, "status": int(info[0]), "sweeps": int(info[1]),
+                                 "scope": "filter+project+device eigensolve+rotate (sparc_gpu_chefsi_step_host_solve)"}
+            del mats_s
         del host_psi, Q_host, Hs_host, Ms_host, mats
         if hasattr(torch._C, "_host_emptyCache"):
             torch._C._host_emptyCache()           # hand the pinned block back to the OS (the next workload sizes its own)
@@ -570,8 +591,8 @@ def bench_shard(env, config, steps, warmup, col_block=0):
         "value": units / (filt * 1e-3), "ms_per_step": step_ms, "scaling": "strong",
         "config": {"workload": wl.name, "grid": list(wl.n), "nd": nd, "ns": ns, "degree": m, "atoms": wl.n_atoms,
                    "col_block": col_block, "stencil_path": g.get_info("stencil_path_last"),
-                   "parallelism": f"shard x{world}: filter by columns, all-to-all, project / rotate by rows, all-reduce of Hs, Ms "
-                                  "(NCCL)",
+                   "parallelism": f"shard x{world}: filter by columns with the all-to-all of each finished block overlapped, "
+                                  "project / rotate by rows, all-reduce of Hs, Ms (NCCL)",
                    "l2": "each rank's slice is larger than the 126 MB L2 and is regenerated between steps"},
         "hbm_gbs": units / (filt * 1e-3) * ALG_BYTES_PER_UNIT / 1e9,
         "subspace_tflops": 3 * 2.0 * nd * ns * ns / ((phase[2] + phase[4]) * 1e-3) / 1e12,
@@ -684,6 +705,10 @@ def run_ours(args):
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     if world > 1:
+        # NCCL's init lines (communicator size, NVLS / ring choice) on stderr, so that a scaling run can be checked for the
+        # rank count and the transport it really used; INIT only, to keep the log short
+        os.environ.setdefault("NCCL_DEBUG", "INFO")
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
         dist.init_process_group("nccl", device_id=dev)
 
     from paper_2302_09708_b200 import api, workloads as wlmod
@@ -762,7 +787,7 @@ def run_ours(args):
             "step_ms": res["step_ms"],
             "filter_frac_of_binding": fr.get("frac_of_binding"), "filter_binding": fr.get("binding"),
             "clocks": short(res["clocks"], ("sm_mhz", "sm_min_mhz", "sm_max_mhz", "power_w_max", "samples", "reasons", "rejected")),
-            "e2e": short(res["e2e"], ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "columns", "step_s", "scope")),
+            "e2e": short(res["e2e"], ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "columns", "step_s", "scope", "with_solve")),
             "gpu_launches": res["gpu_launches"],
             "roofline": roof,
             "cpu_baseline": short(res["cpu_baseline"], ("value", "unit", "cores", "kind", "sample")),

@@ -97,12 +97,14 @@ def barrier(device=None) -> None:
 FORCE_COLLECTIVES = False      # tests: issue the collectives even in a one-rank group (exercises NCCL on a single GPU)
 
 
-def _a2a(recv, send, out_splits, in_splits):
+def _a2a(recv, send, out_splits, in_splits, async_op: bool = False):
+    """all-to-all of flat buffers.  async_op: returns the collective's work handle (None when no collective was issued);
+    the caller keeps `send` / `recv` alive and calls .wait() before it touches `recv`."""
     import torch.distributed as dist
     if _world()[0] == 1 and not (FORCE_COLLECTIVES and dist.is_initialized()):
         recv.copy_(send)
-    else:
-        dist.all_to_all_single(recv, send, output_split_sizes=out_splits, input_split_sizes=in_splits)
+        return None
+    return dist.all_to_all_single(recv, send, output_split_sizes=out_splits, input_split_sizes=in_splits, async_op=async_op)
 
 
 def _block_counts(ns: int, p: int, j0: int, j1: int) -> List[int]:
@@ -114,9 +116,11 @@ def _block_counts(ns: int, p: int, j0: int, j1: int) -> List[int]:
     return out
 
 
-def block_columns_to_rows(Xb, nd: int, ns: int, j0: int, j1: int):
+def block_columns_to_rows(Xb, nd: int, ns: int, j0: int, j1: int, async_op: bool = False):
     """Xb: (nb_me, ld >= nd) = this rank's local columns [j0, j1) (clipped to what it owns).  Returns the (sum_s nb_s, r_me)
-    tensor of this rank's rows of the same local column range of EVERY rank, grouped by source rank."""
+    tensor of this rank's rows of the same local column range of EVERY rank, grouped by source rank, and
+    the per-rank column counts.  async_op: the all-to-all is only started; a third value (work handle or None, send buffer)
+    is returned and the caller waits on the handle before reading the tensor."""
     import torch
     p, me = _world()
     rows = partition_all(nd, p)
@@ -126,7 +130,9 @@ def block_columns_to_rows(Xb, nd: int, ns: int, j0: int, j1: int):
     assert Xb.shape[0] == nb_me
     send = torch.cat([Xb[:, b:e].reshape(-1) for b, e in rows]) if nb_me > 0 else Xb.new_empty(0)
     recv = Xb.new_empty(sum(nbs) * r_me)
-    _a2a(recv, send, [n * r_me for n in nbs], [nb_me * (e - b) for b, e in rows])
+    work = _a2a(recv, send, [n * r_me for n in nbs], [nb_me * (e - b) for b, e in rows], async_op=async_op)
+    if async_op:
+        return recv.view(sum(nbs), r_me), nbs, (work, send)
     return recv.view(sum(nbs), r_me), nbs
 
 
@@ -235,10 +241,35 @@ def chefsi_step(local, Xc, nd: int, ns: int, degree: int, a: float, b: float, a0
     c_max = cols[0][1] - cols[0][0]
     cbk = col_block if col_block > 0 else 1024
     mark("start")
-    if c_me > 0:
-        local.filter(Xc, degree, a, b, a0, col_block)
-    mark("filter")
-    Xr = columns_to_rows(Xc, nd, ns, cbk)
+    # Filter and redistribution, pipelined by column blocks (columns are independent in the filter): the
+    # all-to-all of block j is started asynchronously (it runs on the process group's own stream) and the filter of block
+    # j + 1 is queued behind it on the compute stream, so the NVLink transfer of one block hides under the kernels of the
+    # next.  At most two blocks' send / receive buffers are alive at a time.  The filter's result does not depend on how
+    # its columns are blocked (R19), so this equals filtering the whole slice first.
+    Xr = Xc.new_empty((ns, r_me))
+
+    def finish(item):
+        j0, blk, nbs, (work, _send) = item
+        if work is not None:
+            work.wait()
+        off = 0
+        for s in range(p):
+            Xr[cols[s][0] + j0: cols[s][0] + j0 + nbs[s]].copy_(blk[off:off + nbs[s]])
+            off += nbs[s]
+
+    pending = None
+    for j0 in range(0, c_max, cbk):            # the same number of collectives on every rank
+        j1 = min(j0 + cbk, c_max)
+        Xb = Xc[min(j0, c_me):min(j1, c_me)]
+        if Xb.shape[0] > 0:
+            local.filter(Xb, degree, a, b, a0, col_block)
+        cur = (j0,) + block_columns_to_rows(Xb, nd, ns, j0, j1, async_op=True)
+        if pending is not None:
+            finish(pending)
+        pending = cur
+    if pending is not None:
+        finish(pending)
+    mark("filter")                             # filter and redistribution overlap: "to_rows" is what is left exposed
     mark("to_rows")
     # H~ = sum_k X~^(k)T Y~^(k) by column blocks of Y = H X: a block is formed in the column partition, redistributed and
     # contracted with the whole local row block; column j of Hs is row j of the (ns, ns) tensor

@@ -1,4 +1,4 @@
-"""The N > 1 data path (paper_2302_09708_b200/dist.py) on CPU with two gloo processes: the paper's column / row partitions
+"""The N > 1 data path (paper_2302_09708_b200/dist.py) on CPU with two and with three gloo processes: the paper's column / row partitions
 (PAPER.md:104-108), the column <-> row redistributions, the all-reduce of the partial subspace
 matrices and the whole distributed step, with the local kernels replaced by the oracle (the CUDA kernels
 need a GPU; tests may call oracle/) and the result compared with the single-process oracle."""
@@ -104,7 +104,7 @@ def _worker(rank, world, port, out):
         times = pdist.max_over_ranks([1.0 + rank, 5.0 - rank])
         units = pdist.sum_over_ranks([3.0 + rank])
         # redistribution round trip on a labelled block: element (i, j) = i + 10000 j
-        nd, ns = 37, 5
+        nd, ns = 37, 5                       # world 3: rows 13 + 13 + 11, columns 2 + 2 + 1
         cb, ce = pdist.partition(ns, world, rank)
         rb, re_ = pdist.partition(nd, world, rank)
         full = (np.arange(nd)[:, None] + 10000.0 * np.arange(ns)[None, :])
@@ -135,13 +135,15 @@ def _worker(rank, world, port, out):
         dist.destroy_process_group()
 
 
-def test_two_rank_gloo_step_matches_single_process_oracle():
+@pytest.mark.parametrize("world", [2, 3])
+def test_gloo_step_matches_single_process_oracle(world):
+    """world 2: 7 orbitals as 4 + 3; world 3: 3 + 3 + 1 (ragged last rank), 37 labelled rows as 13 + 13 + 11."""
     import torch.multiprocessing as mp
     from oracle import oracle as orc
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
     port = _free_port()
-    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    procs = [ctx.Process(target=_worker, args=(r, world, port, q)) for r in range(world)]
     for p in procs:
         p.start()
     res = sorted((q.get(timeout=300) for _ in procs), key=lambda t: t[0])
@@ -149,8 +151,8 @@ def test_two_rank_gloo_step_matches_single_process_oracle():
         p.join(timeout=60)
         assert p.exitcode == 0
     for rank, times, units, rows_ok, round_ok, _, _ in res:
-        assert times == [2.0, 5.0]           # max over ranks of [1, 5] and [2, 4]
-        assert units == [7.0]
+        assert times == [float(world), 5.0]   # max over ranks of [1 + rank, 5 - rank]
+        assert units == [3.0 * world + world * (world - 1) / 2]
         assert rows_ok and round_ok
     # single-process reference: filter -> project -> (Q | solve) -> rotate
     wl = _make_wl()
@@ -168,7 +170,8 @@ def test_two_rank_gloo_step_matches_single_process_oracle():
             Hs, Ms = r[6][mode][1], r[6][mode][2]
             assert np.linalg.norm(Hs - Hs_o) <= 1e-12 * np.linalg.norm(Hs_o)
             assert np.linalg.norm(Ms - Ms_o) <= 1e-12 * np.linalg.norm(Ms_o)
-        assert np.array_equal(res[0][6][mode][1], res[1][6][mode][1])    # the all-reduced matrices are the same on both ranks
+        for r in res[1:]:                                                # the all-reduced matrices are the same on every rank
+            assert np.array_equal(res[0][6][mode][1], r[6][mode][1])
         if mode == "given_q":
             assert np.linalg.norm(got - R_given) <= 1e-12 * np.linalg.norm(R_given)
         else:

@@ -138,10 +138,11 @@ def test_chefsi_step_without_host_hop(torch, api):
     gg.close()
 
 
-@pytest.mark.parametrize("n", [256, 1024])
+@pytest.mark.parametrize("n", [256, 1024, 2048, 4096])
 def test_eigensolve_subspace_sizes(torch, api, g, n):
-    """configs[1]'s subspace size (256) and 1024 (configs[2]): validity checks + LAPACK eigenvalues (the oracle's long double
-    Jacobi takes minutes at 1024), with the device time."""
+    """The subspace sizes of configs[1] (256), configs[2] (1024) and configs[3] (4096), and 2048 in between: validity checks
+    (residual, M-orthonormality, ascending D) + LAPACK eigenvalues (the oracle's long double Jacobi takes minutes at 1024),
+    with the device time.  configs[4]'s 7680 is beyond what the Jacobi solver does in useful time."""
     import scipy.linalg as sl
     rng = np.random.default_rng(n)
     H, M = rand_pencil(n, rng, cond=1e2)
