@@ -294,55 +294,6 @@ class SparcGpu:
                "chebyshev_filter")
         return Psi
 
-    def chebyshev_filter_host(self, host_in, host_out, degree: int, a: float, b: float, a0: float,
-                              chunk_cols: int = 0, col_block: int = 0):
-        """Filter a block that lives in PINNED HOST memory: host_in (ncols, ld) -> host_out (same shape).
-
-        Plumbing only: the columns are independent, so the block is cut into column chunks that are
-        copied in, filtered by `sparc_gpu_chebyshev_filter` and copied out on three CUDA streams, so that the PCIe
-        transfers of neighbouring chunks overlap the kernels.  Synchronises before returning."""
-        torch = _torch()
-        assert host_in.is_pinned() and host_out.is_pinned() and host_in.shape == host_out.shape
-        assert host_in.dtype == torch.float64 and host_in.dim() == 2 and host_in.stride(1) == 1
-        ns, ld = int(host_in.shape[0]), int(host_in.shape[1])
-        if ns == 0:
-            return host_out
-        dev = torch.device("cuda", self.device)
-        if chunk_cols <= 0:       # >= 64 MB and >= 64 columns per chunk (PCIe and launch efficiency), else as many chunks as fit
-            chunk_cols = max(1, min(ns, max(64, (64 << 20) // (ld * 8))))
-        nbuf = 3
-        bufs = [torch.empty((min(chunk_cols, ns), ld), dtype=torch.float64, device=dev) for _ in range(nbuf)]
-        self._workspace(OP_CHEBYSHEV_FILTER, min(chunk_cols, ns), col_block)      # allocate once, before the streams
-        s_in, s_run, s_out = (torch.cuda.Stream(device=dev) for _ in range(3))
-        start = torch.cuda.Event()
-        start.record()
-        for st in (s_in, s_run, s_out):
-            st.wait_event(start)
-        out_done = []
-        for i, j0 in enumerate(range(0, ns, chunk_cols)):
-            nb = min(chunk_cols, ns - j0)
-            buf = bufs[i % nbuf][:nb]
-            with torch.cuda.stream(s_in):
-                if i >= nbuf:
-                    s_in.wait_event(out_done[i - nbuf])          # the buffer's previous chunk has left the device
-                buf.copy_(host_in[j0:j0 + nb], non_blocking=True)
-                ev_in = torch.cuda.Event()
-                ev_in.record(s_in)
-            with torch.cuda.stream(s_run):
-                s_run.wait_event(ev_in)
-                self.chebyshev_filter(buf, degree, a, b, a0, col_block=col_block)
-                ev_run = torch.cuda.Event()
-                ev_run.record(s_run)
-            with torch.cuda.stream(s_out):
-                s_out.wait_event(ev_run)
-                host_out[j0:j0 + nb].copy_(buf, non_blocking=True)
-                ev_out = torch.cuda.Event()
-                ev_out.record(s_out)
-            out_done.append(ev_out)
-        for st in (s_in, s_run, s_out):
-            st.synchronize()
-        return host_out
-
     def chefsi_step_host(self, host_psi, Q_host, Hs_host, Ms_host, degree: int, a: float, b: float, a0: float,
                          psi_dev=None, mats_dev=None, col_block: int = 0, row_panel: int = 0, host_out=None):
         """sparc_gpu_chefsi_step_host: filter -> project -> rotate on a block in (pinned) HOST memory.  host_psi:

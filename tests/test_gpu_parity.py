@@ -366,23 +366,6 @@ def test_lower_fd_orders(torch, api, fd_order):
     g.close()
 
 
-def test_filter_host_buffers_pipelined(torch, api):
-    """The host-buffer path (column chunks pipelined over three streams) gives the same block as the oracle."""
-    pos = np.array([[1.0, 2.0, 3.0], [4.0, 1.0, 0.5]])
-    wl = wlmod.make_custom("hostpipe", (16, 18, 14), (0.4, 0.4, 0.45), (0, 0, 1), 13, 5, pos, [4, 9], 2.2, seed=17)
-    g = api.SparcGpu(wl)
-    X = wl.psi_columns(range(wl.ns))
-    hin = torch.from_numpy(np.ascontiguousarray(X.T)).pin_memory()
-    hout = torch.empty_like(hin).pin_memory()
-    for chunk in (5, 0):
-        hout.zero_()
-        g.chebyshev_filter_host(hin, hout, wl.degree, wl.a, wl.b, wl.a0, chunk_cols=chunk)
-        check_col(np.asfortranarray(hout.numpy().T), orc.Hamiltonian(wl).chebyshev_filter(X, wl.degree, wl.a, wl.b, wl.a0),
-                  f"host-buffer filter, chunk_cols={chunk}")
-    assert np.array_equal(hin.numpy().T, X)
-    g.close()
-
-
 def test_degenerate_calls(torch, api):
     wl = wlmod.make_workload(0)
     g = api.SparcGpu(wl)
