@@ -165,6 +165,47 @@ def test_kpoint_config1_sampled(torch, api):
     g.close()
 
 
+def test_kpoint_config2_grid_256_orbitals_sampled(torch, api):
+    """configs[2]'s grid and atoms (60 x 60 x 180 slab, Dirichlet z) with 256 complex orbitals, the block generated on the
+    device (same counter-based generator as the host's): filter on sampled columns, Hermitian products on sampled entries and
+    the rotation on sampled rows against the oracle -- the k-point path at a size where the column blocking, the real-view
+    GEMMs and the row panels all take several tiles."""
+    wl = wlmod.make_workload(2)
+    ns, nd = 256, wl.nd
+    theta = np.array([0.5 * np.pi, 0.25 * np.pi, 0.0])
+    g = api.SparcGpu(wl)
+    g.set_kpoint(theta, wl.supp_shift)
+    re = torch.empty((ns, nd), dtype=torch.float64, device="cuda")
+    im = torch.empty_like(re)
+    api.fill_uniform(re, wl.seed, wlmod.STREAM_PSI, 0, -1.0, 1.0)
+    api.fill_uniform(im, wl.seed, wlmod.STREAM_PSI_IMAG, 0, -1.0, 1.0)
+    Pg = torch.complex(re, im)
+    del re, im
+    cols = [0, 100, 255]
+    X = wl.psi_columns_complex(cols)
+    assert np.array_equal(to_host(Pg[cols]), X)               # the two generators agree bit for bit
+    g.chebyshev_filter_k(Pg, wl.degree, wl.a, wl.b, wl.a0)
+    Hk = orc.HamiltonianK(wl, theta)
+    Fo = Hk.chebyshev_filter(X, wl.degree, wl.a, wl.b, wl.a0)
+    Fg = to_host(Pg[cols])
+    e = col_err(Fg, Fo)
+    print(f"[parity] cfg2-grid k-point filter, 256 orbitals, sampled columns: {e:.2e}")
+    assert e <= 1e-10 and e <= 1e-13
+    Hs, Ms = g.project_k(Pg)
+    Hs_o = orc.gram_k(Fg, Hk.apply(Fg))
+    Ms_o = orc.gram_k(Fg, Fg)
+    assert fro_err(to_host(Hs)[np.ix_(cols, cols)], Hs_o) <= 1e-11
+    assert fro_err(to_host(Ms)[np.ix_(cols, cols)], Ms_o) <= 1e-11
+    rows = np.array([0, 59, 3600, 300000, nd - 1])
+    before = np.ascontiguousarray(Pg[:, torch.from_numpy(rows).cuda()].cpu().numpy().T)      # (rows, ns)
+    rng = np.random.default_rng(4)
+    Q = np.linalg.qr(rng.normal(size=(ns, ns)) + 1j * rng.normal(size=(ns, ns)))[0]
+    g.rotate_k(Pg, to_dev(torch, Q))
+    after = np.ascontiguousarray(Pg[:, torch.from_numpy(rows).cuda()].cpu().numpy().T)
+    assert fro_err(after, orc.rotate_k(before, Q)) <= 1e-11
+    g.close()
+
+
 def test_kpoint_lower_fd_order(torch, api):
     """FD order 4 (radius 2) on a short periodic grid: wrapped taps with their phases for a stencil narrower than the maximum."""
     pos = np.array([[1.0, 2.0, 1.5]])
